@@ -1,0 +1,188 @@
+"""oracle — ctypes access to the CPU oracle (TEST INFRASTRUCTURE, not the product).
+
+Only tests/, ``__graft_entry__.smoke()`` and bench.py's cpu_baseline / ``--impl reference`` leg may import
+this.  It never imports ``paper_2211_14346_b200`` and the CUDA package never imports it.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libhepf_oracle.so")
+_SRCS = ["oracle_philox.cpp", "oracle_select.cpp", "oracle_reco.cpp"]
+
+
+def build(force: bool = False) -> str:
+    srcs = [os.path.join(_HERE, s) for s in _SRCS]
+    deps = srcs + [os.path.join(_HERE, "hepf_oracle.h")]
+    if force or not os.path.exists(_LIB_PATH) or os.path.getmtime(_LIB_PATH) < max(map(os.path.getmtime, deps)):
+        subprocess.check_call(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+                               "-Wall", "-o", _LIB_PATH] + srcs)
+    return _LIB_PATH
+
+
+class Events(C.Structure):
+    _fields_ = [("n_events", C.c_int64), ("stride", C.c_int64), ("event_base", C.c_int64)] + \
+               [(n, C.c_void_p) for n in ("lep_px", "lep_py", "lep_pz", "lep_e", "lep_pt", "lep_eta",
+                                          "jet_px", "jet_py", "jet_pz", "jet_e", "jet_pt", "jet_eta",
+                                          "met_x", "met_y", "met", "mll", "flags")]
+
+
+class Cut(C.Structure):
+    _fields_ = [("kind", C.c_uint32), ("n", C.c_uint32), ("lo", C.c_double), ("hi", C.c_double)]
+
+
+class Params(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("m_top", "m_w", "m_higgs", "sigma_higgs", "lambda_nu", "lep_sigma",
+                                          "jet_stoch", "jet_const", "sigma_scale", "s_min")]
+
+
+BEST_DTYPE = np.dtype([("nu", "f8", 3), ("nubar", "f8", 3), ("m_top", "f8"), ("m_antitop", "f8"),
+                       ("m_wplus", "f8"), ("m_wminus", "f8"), ("m_higgs", "f8"), ("loglik", "f8"),
+                       ("variation", "i4"), ("jet_b", "i4"), ("jet_bbar", "i4"), ("jet_h1", "i4"),
+                       ("jet_h2", "i4"), ("root", "i4"), ("status", "u4"), ("event", "u4")])
+AUX_DTYPE = np.dtype([("kappa", "f8"), ("loglik2", "f8"), ("n_cand", "i8"), ("pairing", "i4"),
+                      ("higgs_pair", "i4")])
+assert BEST_DTYPE.itemsize == 128 and AUX_DTYPE.itemsize == 32
+
+
+class Pairing(C.Structure):
+    _fields_ = [("n_roots", C.c_int32), ("n_higgs", C.c_int32), ("g", C.c_double * 4), ("h", C.c_double * 5),
+                ("conic1", C.c_double * 6), ("conic2", C.c_double * 6), ("x", C.c_double * 4),
+                ("kappa", C.c_double * 4), ("nterm", C.c_double * 4), ("nu", (C.c_double * 4) * 4),
+                ("nubar", (C.c_double * 4) * 4), ("hterm", C.c_double * 6), ("mbb", C.c_double * 6),
+                ("min_abs_p_rel", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.orc_det_log.restype = C.c_double
+        L.orc_det_log.argtypes = [C.c_double]
+        L.orc_det_sincos2pi.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.orc_philox_normal.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p]
+        L.orc_philox_normal.restype = None
+        L.orc_select.argtypes = [C.POINTER(Events), C.POINTER(Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_reconstruct_tth.argtypes = [C.POINTER(Events), C.c_void_p, C.c_int64, C.c_int32, C.c_uint64,
+                                          C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_int]
+        L.orc_solve_pairing.argtypes = [C.c_void_p] * 6 + [C.c_int, C.POINTER(Params), C.POINTER(Pairing)]
+        L.orc_eval_cell.argtypes = [C.POINTER(Events), C.c_uint32, C.c_int32, C.c_int32, C.c_uint64,
+                                    C.POINTER(Params), C.POINTER(Pairing)]
+        L.orc_smear.argtypes = [C.POINTER(Events), C.c_uint32, C.c_int32, C.c_uint64, C.POINTER(Params),
+                                C.c_void_p, C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def default_params(**over) -> Params:
+    p = Params()
+    lib().orc_default_params(C.byref(p))
+    for k, v in over.items():
+        setattr(p, k, v)
+    return p
+
+
+def events_view(store) -> Events:
+    """View of a host EventStore (hepf_synth.EventStore: cols[64, stride] float64, flags[stride] uint32)."""
+    from hepf_synth import ROW
+    ev = Events()
+    ev.n_events, ev.stride, ev.event_base = store.n_events, store.stride, store.event_base
+    base, rb = store.cols.ctypes.data, store.stride * 8
+    for name, row in ROW.items():
+        setattr(ev, name, base + row * rb)
+    ev.flags = store.flags.ctypes.data
+    ev._keep = store
+    return ev
+
+
+def make_cuts(chain):
+    arr = (Cut * max(1, len(chain)))()
+    for i, (kind, n, lo, hi) in enumerate(chain):
+        arr[i] = Cut(kind, n, lo, hi)
+    return arr
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr); k = (C.c_uint32 * 2)(*key); o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return list(o)
+
+
+def det_log(u: float) -> float:
+    return lib().orc_det_log(u)
+
+
+def det_sincos2pi(u: float):
+    s, c = C.c_double(), C.c_double()
+    lib().orc_det_sincos2pi(u, C.byref(s), C.byref(c))
+    return s.value, c.value
+
+
+def philox_normal(seed: int, counter: int, n: int) -> np.ndarray:
+    out = np.empty(n, dtype=np.float64)
+    lib().orc_philox_normal(seed, counter, n, out.ctypes.data)
+    return out
+
+
+def select(store, chain):
+    ev = events_view(store)
+    idx = np.empty(store.n_events, dtype=np.uint32)
+    count = np.zeros(1, dtype=np.int64)
+    cutflow = np.zeros(max(1, len(chain)), dtype=np.int64)
+    rc = lib().orc_select(C.byref(ev), make_cuts(chain), len(chain), idx.ctypes.data, count.ctypes.data,
+                          cutflow.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_select: {rc}")
+    return idx[: int(count[0])].copy(), cutflow[: len(chain)].copy()
+
+
+def reconstruct_tth(store, idx, n_variations: int, seed: int, params: Params | None = None, n_threads: int = 1):
+    ev = events_view(store)
+    idx = np.ascontiguousarray(idx, dtype=np.uint32)
+    best = np.zeros(len(idx), dtype=BEST_DTYPE)
+    aux = np.zeros(len(idx), dtype=AUX_DTYPE)
+    rc = lib().orc_reconstruct_tth(C.byref(ev), idx.ctypes.data, len(idx), n_variations, seed,
+                                   C.byref(params) if params is not None else None, best.ctypes.data,
+                                   aux.ctypes.data, n_threads)
+    if rc != 0:
+        raise RuntimeError(f"orc_reconstruct_tth: {rc}")
+    return best, aux
+
+
+def solve_pairing(lp, b, lm, bbar, met, jets_h=(), params: Params | None = None) -> Pairing:
+    arrs = [np.ascontiguousarray(a, dtype=np.float64) for a in (lp, b, lm, bbar, met)]
+    jh = np.ascontiguousarray(np.asarray(jets_h, dtype=np.float64).reshape(-1, 4)) if len(jets_h) else np.zeros((0, 4))
+    out = Pairing()
+    rc = lib().orc_solve_pairing(*[a.ctypes.data for a in arrs], jh.ctypes.data, len(jh),
+                                 C.byref(params) if params is not None else None, C.byref(out))
+    if rc != 0:
+        raise RuntimeError(f"orc_solve_pairing: {rc}")
+    return out
+
+
+def eval_cell(store, e: int, v: int, a: int, seed: int, params: Params | None = None) -> Pairing:
+    ev = events_view(store)
+    out = Pairing()
+    rc = lib().orc_eval_cell(C.byref(ev), e, v, a, seed, C.byref(params) if params is not None else None,
+                             C.byref(out))
+    if rc < 0:
+        raise RuntimeError(f"orc_eval_cell: {rc}")
+    return out
+
+
+def smear(store, e: int, v: int, seed: int, params: Params | None = None):
+    ev = events_view(store)
+    s = np.zeros(10); m = np.zeros(2)
+    rc = lib().orc_smear(C.byref(ev), e, v, seed, C.byref(params) if params is not None else None,
+                         s.ctypes.data, m.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_smear: {rc}")
+    return s, m

@@ -1,0 +1,106 @@
+/*
+ * oracle/hepf_oracle.h — CPU ORACLE (TEST INFRASTRUCTURE, NOT THE PRODUCT).
+ *
+ * Plain, slow, obviously-correct FP64 restatement of the ttH hot path of arXiv 2211.14346 (HEP-Frame),
+ * §4 "ttH case study": ordered boolean cuts, then per
+ * event x smearing variation x b-jet/lepton pairing the analytic dilepton neutrino reconstruction with
+ * m_W = 80.4, m_t = 172.5 and the Higgs pair at 125 GeV, "highest probability" wins.
+ * The paper gives no equations (they are in its ref. [27]); the step-by-step definition followed here is
+ * SURVEY.md §8(c) O1-O4 with the readings R1-R13 listed in DESIGN.md.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may use this
+ * library.  It shares no code, header, table or constant generator with the CUDA path under
+ * paper_2211_14346_b200/csrc: the struct definitions below are this tree's own declarations.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"):
+ *   O1 Philox4x32-10 ......... known-answer vectors (tests/golden/philox_kat.txt)
+ *   O2 uniforms / normals .... six printed hex-float normals, slice consistency, moments,
+ *                              det-log / det-sincos against libm within 4 ulp
+ *   O3 select ................ hand-built threshold tables, numpy restatement, cutflow invariants
+ *   O4 conic/quartic algebra . worked example (tests/golden/worked_example.txt), closure invariant,
+ *                              truth recovery in closure mode, multi-start Newton brute force on the
+ *                              raw mass constraints, dense-grid sign-change brute force on the quartic
+ *   O4 score / argmax ........ prefix property in V, sigma_scale = 0, z-rotation invariance, slot permutation
+ *   PARITY UNPINNED against the paper: the likelihood formula, sigma_H, lambda_nu, the resolution model
+ *   and the 8-cut thresholds are definitions of this build (R3, R7, R10), not paper values.
+ */
+#ifndef HEPF_ORACLE_H
+#define HEPF_ORACLE_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+  int64_t n_events, stride, event_base;
+  const double *lep_px, *lep_py, *lep_pz, *lep_e, *lep_pt, *lep_eta; /* [2][stride] */
+  const double *jet_px, *jet_py, *jet_pz, *jet_e, *jet_pt, *jet_eta; /* [8][stride] */
+  const double *met_x, *met_y, *met, *mll;                           /* [stride]    */
+  const uint32_t* flags;
+} orc_events_t;
+
+typedef struct { uint32_t kind, n; double lo, hi; } orc_cut_t;
+enum { ORC_NLEP_EQ = 1, ORC_LEP_OS, ORC_LEP_PT_GT, ORC_LEP_ABSETA_LT, ORC_NJET_GE, ORC_NBJET_GE, ORC_MET_GT,
+       ORC_MLL_GT, ORC_MLL_OUTSIDE };
+
+typedef struct {
+  double m_top, m_w, m_higgs, sigma_higgs, lambda_nu, lep_sigma, jet_stoch, jet_const, sigma_scale, s_min;
+} orc_params_t;
+
+typedef struct {
+  double nu[3], nubar[3];
+  double m_top, m_antitop, m_wplus, m_wminus, m_higgs, loglik;
+  int32_t variation, jet_b, jet_bbar, jet_h1, jet_h2, root;
+  uint32_t status, event;
+} orc_best_t;
+
+typedef struct {      /* per-event diagnostics the parity harness needs (R11) */
+  double kappa;       /* eps * sum|h_i x^i| / |x P'(x)| of the winning root            */
+  double loglik2;     /* best log-likelihood among all other candidates (-inf if none)  */
+  int64_t n_cand;     /* candidates enumerated                                          */
+  int32_t pairing, higgs_pair; /* a = i*n_b + j and h of the winner                     */
+} orc_aux_t;
+
+typedef struct {      /* one pairing solved in isolation (worked example, brute-force pins, R11 ii/iii) */
+  int32_t n_roots, n_higgs;
+  double g[4];        /* monic quartic x^4 + g3 x^3 + g2 x^2 + g1 x + g0: g[0]=g0 .. g[3]=g3 */
+  double h[5];        /* raw resultant coefficients h0..h4                                    */
+  double conic1[6], conic2[6]; /* a b c d e f; conic2 already shifted by MET'                 */
+  double x[4], kappa[4], nterm[4];
+  double nu[4][4], nubar[4][4];  /* px py pz E per root                                        */
+  double hterm[6], mbb[6];
+  double min_abs_p_rel; /* min over critical points of |P|/sum|h_i x^i| (near-tangency measure) */
+} orc_pairing_t;
+
+void orc_default_params(orc_params_t* p);
+
+/* O1 */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* O2 */
+double orc_det_log(double u);
+void orc_det_sincos2pi(double u, double* s, double* c);
+void orc_philox_normal(uint64_t seed, uint64_t counter, uint64_t n, double* out);
+/* O3 */
+int orc_select(const orc_events_t* ev, const orc_cut_t* cuts, int n_cuts, uint32_t* out_idx, int64_t* out_count,
+               int64_t* out_cutflow);
+/* O4: n_threads > 1 only distributes whole events over OpenMP threads; per-event arithmetic is unchanged */
+int orc_reconstruct_tth(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
+                        uint64_t seed, const orc_params_t* params, orc_best_t* out_best, orc_aux_t* out_aux,
+                        int n_threads);
+/* one pairing from explicit four-vectors (px,py,pz,E); jets_h = n_h remaining b candidates (<= 4) */
+int orc_solve_pairing(const double lp[4], const double b[4], const double lm[4], const double bbar[4],
+                      const double met[2], const double* jets_h, int n_h, const orc_params_t* params,
+                      orc_pairing_t* out);
+/* the (event, variation, pairing a) cell of orc_reconstruct_tth, re-evaluated on request */
+int orc_eval_cell(const orc_events_t* ev, uint32_t e, int32_t v, int32_t a, uint64_t seed,
+                  const orc_params_t* params, orc_pairing_t* out);
+/* smeared objects of one (event, variation): scales[10], met'[2] */
+int orc_smear(const orc_events_t* ev, uint32_t e, int32_t v, uint64_t seed, const orc_params_t* params,
+              double scales[10], double metp[2]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
