@@ -1,0 +1,161 @@
+/*
+ * include/hepf.h — C ABI of libhepf: the ttH selection + kinematic-reconstruction hot path of
+ * arXiv 2211.14346 (HEP-Frame, §4 "ttH case study") as hand-written CUDA for sm_100a (one B200 per process).
+ *
+ * Conventions (all entry points)
+ *   - plain C types only; no exceptions cross the boundary.
+ *   - "device" pointers are caller-owned device memory (e.g. torch tensors); "host" pointers are ordinary
+ *     host memory read during the call.  The library never allocates or frees device memory: scratch space
+ *     is a caller-provided workspace whose size the *_workspace_bytes functions return.
+ *   - every device entry point only ENQUEUES work on `stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream) and returns; results are valid after the caller synchronises that stream.
+ *     hepf_tth_host is the exception: it takes host buffers and returns after its results are on the host.
+ *   - return value: HEPF_OK or a negative error code; hepf_last_error() gives a host string (thread-local)
+ *     for the last failure.  On error nothing is guaranteed about the output buffers.
+ *   - there is NO CPU fallback: without a CUDA device every compute entry point returns HEPF_ERR_CUDA.
+ *   - units GeV; FP64 throughout ("dtype f64").
+ */
+#ifndef HEPF_H
+#define HEPF_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HEPF_OK 0
+#define HEPF_ERR_ARG (-1)      /* null / misaligned pointer, negative size, n_cuts > 32, n_variations < 1, odd stride */
+#define HEPF_ERR_CAPACITY (-2) /* workspace or arena too small                                                    */
+#define HEPF_ERR_CUDA (-3)     /* CUDA runtime / launch failure, or no device                                     */
+
+#define HEPF_MAX_CUTS 32
+#define HEPF_N_LEP 2
+#define HEPF_N_JET 8
+#define HEPF_MAX_B 6
+
+/*
+ * SoA event store: a VIEW of caller-owned columns (§3: all in-flight events are kept in
+ * memory by the framework and are visible to every cut).  Column c of object slot s lives at
+ * ptr[s * stride + event].  Leptons and jets are pT-ordered; unused slots hold zeros.
+ *   stride      >= n_events, even (so that every slot row is 16-byte aligned); every pointer 16-byte aligned.
+ *   event_base  global index of event 0 of this view: the smearing stream of event e is keyed by
+ *               event_base + e, so results do not depend on how a sample is split into views / ranks.
+ *   flags       bits 0-3 n_lep | bit 4 q(lep0) > 0 | bit 5 q(lep1) > 0 | bits 8-11 n_jet | bits 16-23 b-tag mask.
+ */
+typedef struct {
+  int64_t n_events, stride, event_base;
+  const double *lep_px, *lep_py, *lep_pz, *lep_e, *lep_pt, *lep_eta; /* [2][stride] */
+  const double *jet_px, *jet_py, *jet_pz, *jet_e, *jet_pt, *jet_eta; /* [8][stride] */
+  const double *met_x, *met_y, *met, *mll;                           /* [stride]    */
+  const uint32_t* flags;                                             /* [stride]    */
+} hepf_events_t;
+
+/*
+ * One cut of the ordered chain (`bool cut(event)`, registered in order, an event is dropped
+ * at the first false; thresholds are strict — "met <= 30000 -> fail").  A comparison with a
+ * NaN is false, so the event fails.  Jet counts look at slots 0 .. n_jet-1 only.
+ */
+typedef enum {
+  HEPF_CUT_NLEP_EQ = 1,       /* n_lep == n                                            */
+  HEPF_CUT_LEP_OS = 2,        /* lepton charge bits differ                             */
+  HEPF_CUT_LEP_PT_GT = 3,     /* both leptons: pt > lo                                 */
+  HEPF_CUT_LEP_ABSETA_LT = 4, /* both leptons: |eta| < hi                              */
+  HEPF_CUT_NJET_GE = 5,       /* #jets with pt > lo and |eta| < hi  >= n               */
+  HEPF_CUT_NBJET_GE = 6,      /* same, b-tagged jets only                              */
+  HEPF_CUT_MET_GT = 7,        /* met > lo                                              */
+  HEPF_CUT_MLL_GT = 8,        /* mll > lo                                              */
+  HEPF_CUT_MLL_OUTSIDE = 9    /* mll < lo or mll > hi                                  */
+} hepf_cut_kind_t;
+typedef struct { uint32_t kind; uint32_t n; double lo, hi; } hepf_cut_t;
+
+/* Parameters of the reconstruction (NULL = defaults).  m_top, m_w, m_higgs: PAPER.md:138 (172.5, 80.4, 125).
+ * lep_sigma 0.01: PAPER.md:145; jet resolution sigma/E = jet_stoch/sqrt(E) + jet_const (0.5, 0.03):
+ * BASELINE.json configs[0].  sigma_higgs 15, lambda_nu 40, sigma_scale 1, s_min 0.1: definitions of this
+ * build (readings R3-R7). */
+typedef struct {
+  double m_top, m_w, m_higgs, sigma_higgs, lambda_nu, lep_sigma, jet_stoch, jet_const, sigma_scale, s_min;
+} hepf_tth_params_t;
+
+/* Best solution of one event ("the one with highest probability is considered to be the correct
+ * solution"; "only the highest probable solution was considered").  128 bytes.
+ * status bits: 1 = has a solution; 2 = not applicable (n_lep != 2, same-sign, < 4 b candidates);
+ *              4 = more than 6 b candidates, truncated to the 6 lowest slots.
+ * Without a solution the floating-point payload is NaN and the integer payload is -1 (the paper's "discards the
+ * event if no solution was found"). */
+typedef struct {
+  double nu[3], nubar[3];                                        /* neutrino / antineutrino 3-momenta        */
+  double m_top, m_antitop, m_wplus, m_wminus, m_higgs, loglik;   /* recomputed from the output four-vectors  */
+  int32_t variation, jet_b, jet_bbar, jet_h1, jet_h2, root;      /* jet_* are jet slot indices; root = rank  */
+  uint32_t status, event;                                        /* event = idx[k] (index inside the view)   */
+} hepf_best_t;
+
+/*
+ * hepf_select — evaluate the cut chain, one thread per event, and compact the survivors (PAPER.md:96-102,
+ * :122 filtered output, §4 :136 "eighteen cuts, organised in a sequential way").
+ *   events       host pointer to a view of DEVICE columns.
+ *   host_cuts    host array of n_cuts (0..32) cuts, applied in order.
+ *   out_idx      device, capacity n_events: ascending indices of surviving events (stable compaction).
+ *   out_count    device int64: number of survivors.
+ *   out_cutflow  device int64[n_cuts] or NULL: cutflow[c] = events that passed cuts 0..c.
+ *   ws           device workspace of at least hepf_select_workspace_bytes(n_events) bytes, 16-byte aligned.
+ */
+int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
+                int64_t* out_count, int64_t* out_cutflow, void* ws, size_t ws_bytes, void* stream);
+size_t hepf_select_workspace_bytes(int64_t n_events);
+
+/*
+ * hepf_reconstruct_tth — for each listed event: for every smearing variation v < n_variations draw ten
+ * standard normals from Philox4x32-10 keyed (seed; event_base+e, v, block) + Box-Muller, scale the two leptons
+ * and the jets, propagate the change to the missing transverse momentum, and for every ordered pair of b-jet
+ * candidates solve the dileptonic ttbar kinematics (two leg conics -> quartic; Ferrari closed form + Newton
+ * polish, FP64), score every solution (Higgs pair mass term + neutrino pT term) and keep the best over
+ * variations x pairings x Higgs pairs x roots (§4; definition: DESIGN.md "Method").
+ *   idx          device uint32[n_idx]: events to reconstruct (normally hepf_select's out_idx); values < n_events.
+ *   n_idx        host value.
+ *   host_params  host pointer or NULL.
+ *   out_best     device hepf_best_t[n_idx], 16-byte aligned; out_best[k] belongs to idx[k].
+ *   ws           device workspace >= hepf_reconstruct_workspace_bytes(n_idx, n_variations) (may be 0 -> NULL ok).
+ */
+int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
+                         uint64_t seed, const hepf_tth_params_t* host_params, hepf_best_t* out_best, void* ws,
+                         size_t ws_bytes, void* stream);
+size_t hepf_reconstruct_workspace_bytes(int64_t n_idx, int32_t n_variations);
+void hepf_default_params(hepf_tth_params_t* host_params);
+
+/*
+ * hepf_philox_normal — out[i] = Z[counter + i], i < n, of the single infinite stream of standard normals
+ * Z[g]: Philox block b = g >> 1 with counter words (b mod 2^32, b >> 32, 0, 0) and key (seed mod 2^32,
+ * seed >> 32); (Z[2b], Z[2b+1]) = rho (cos, sin)(2 pi u2), rho = sqrt(-2 ln u1) (the exact
+ * operation sequence, identical bits for any split of a range into calls or blocks).  The paper's PRNG
+ * offload: §5.3.   out: device double[n], 8-byte aligned.
+ */
+int hepf_philox_normal(uint64_t seed, uint64_t counter, uint64_t n, double* out, void* stream);
+
+/*
+ * hepf_tth_host — the whole path from HOST buffers: copies the columns of `host_events` (a view of HOST
+ * memory, pinned for full speed) to the device arena, runs hepf_select and hepf_reconstruct_tth and copies the
+ * results back.  Synchronous: returns when host_out_* are filled.
+ *   host_out_idx   host uint32[n_events] or NULL;  host_out_best  host hepf_best_t[n_events] (first n_sel used);
+ *   host_out_count host int64;  host_out_cutflow host int64[n_cuts] or NULL.
+ *   arena          device scratch >= hepf_tth_host_arena_bytes(n_events, n_variations), 256-byte aligned.
+ */
+int hepf_tth_host(const hepf_events_t* host_events, const hepf_cut_t* host_cuts, int n_cuts, int32_t n_variations,
+                  uint64_t seed, const hepf_tth_params_t* host_params, uint32_t* host_out_idx,
+                  hepf_best_t* host_out_best, int64_t* host_out_count, int64_t* host_out_cutflow, void* arena,
+                  size_t arena_bytes, void* stream);
+size_t hepf_tth_host_arena_bytes(int64_t n_events, int32_t n_variations);
+
+/* Kernel launches enqueued by this thread's calls since the last reset (bench.py's `gpu_launches`). */
+int64_t hepf_launch_count(int reset);
+/* FP64 FMA-chain micro-benchmark used to measure the FP64 roof on the box: enqueues one kernel that performs
+ * `fma_per_thread` dependent-chain-of-8 DFMAs per thread over blocks x threads; writes a checksum to `sink`. */
+int hepf_fp64_peak_probe(int blocks, int threads, int64_t fma_per_thread, double* sink, void* stream);
+
+const char* hepf_last_error(void);
+const char* hepf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,11 @@
+"""paper_2211_14346_b200 — B200-native ttH selection + kinematic reconstruction (arXiv 2211.14346, §4).
+
+Thin Python binding over the C ABI of ``libhepf.so`` (``include/hepf.h``): argument marshalling only — every
+step of the path runs in the hand-written sm_100a kernels under ``csrc/``.  PyTorch supplies device memory and
+streams.  There is no CPU fallback: importing works anywhere, calling needs the built library and a CUDA device.
+"""
+from .binding import (BEST_DTYPE, DeviceEvents, HepfError, default_params, fp64_peak_probe, last_error, launch_count,
+                      lib_path, load, make_cuts, philox_normal, reconstruct_tth, select, tth_host)
+
+__all__ = ["BEST_DTYPE", "DeviceEvents", "HepfError", "default_params", "fp64_peak_probe", "last_error",
+           "launch_count", "lib_path", "load", "make_cuts", "philox_normal", "reconstruct_tth", "select", "tth_host"]

@@ -1,0 +1,235 @@
+"""ctypes binding of libhepf.so: same names as the C entry points, marshalling only (include/hepf.h)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = os.path.join(_HERE, "libhepf.so")
+
+# row offsets of the 64-row column block (same layout as the host store the generator writes)
+ROW = dict(lep_px=0, lep_py=2, lep_pz=4, lep_e=6, lep_pt=8, lep_eta=10,
+           jet_px=12, jet_py=20, jet_pz=28, jet_e=36, jet_pt=44, jet_eta=52,
+           met_x=60, met_y=61, met=62, mll=63)
+NROW = 64
+
+BEST_DTYPE = np.dtype([("nu", "f8", 3), ("nubar", "f8", 3), ("m_top", "f8"), ("m_antitop", "f8"),
+                       ("m_wplus", "f8"), ("m_wminus", "f8"), ("m_higgs", "f8"), ("loglik", "f8"),
+                       ("variation", "i4"), ("jet_b", "i4"), ("jet_bbar", "i4"), ("jet_h1", "i4"),
+                       ("jet_h2", "i4"), ("root", "i4"), ("status", "u4"), ("event", "u4")])
+assert BEST_DTYPE.itemsize == 128
+
+
+class HepfError(RuntimeError):
+    pass
+
+
+class _Events(C.Structure):
+    _fields_ = [("n_events", C.c_int64), ("stride", C.c_int64), ("event_base", C.c_int64)] + \
+               [(n, C.c_void_p) for n in ("lep_px", "lep_py", "lep_pz", "lep_e", "lep_pt", "lep_eta",
+                                          "jet_px", "jet_py", "jet_pz", "jet_e", "jet_pt", "jet_eta",
+                                          "met_x", "met_y", "met", "mll", "flags")]
+
+
+class _Cut(C.Structure):
+    _fields_ = [("kind", C.c_uint32), ("n", C.c_uint32), ("lo", C.c_double), ("hi", C.c_double)]
+
+
+class Params(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("m_top", "m_w", "m_higgs", "sigma_higgs", "lambda_nu", "lep_sigma",
+                                          "jet_stoch", "jet_const", "sigma_scale", "s_min")]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB
+
+
+def load():
+    """Load libhepf.so (fails loudly if it has not been built: there is no fallback path)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB):
+            raise HepfError(f"{_LIB} is missing: run `python -m paper_2211_14346_b200.build` "
+                            "(or __graft_entry__.build()) first; there is no CPU fallback")
+        L = C.CDLL(_LIB)
+        L.hepf_last_error.restype = C.c_char_p
+        L.hepf_version.restype = C.c_char_p
+        L.hepf_launch_count.restype = C.c_int64
+        L.hepf_launch_count.argtypes = [C.c_int]
+        L.hepf_select_workspace_bytes.restype = C.c_size_t
+        L.hepf_select_workspace_bytes.argtypes = [C.c_int64]
+        L.hepf_reconstruct_workspace_bytes.restype = C.c_size_t
+        L.hepf_reconstruct_workspace_bytes.argtypes = [C.c_int64, C.c_int32]
+        L.hepf_tth_host_arena_bytes.restype = C.c_size_t
+        L.hepf_tth_host_arena_bytes.argtypes = [C.c_int64, C.c_int32]
+        L.hepf_default_params.argtypes = [C.POINTER(Params)]
+        L.hepf_select.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                  C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hepf_reconstruct_tth.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_int32, C.c_uint64,
+                                           C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hepf_philox_normal.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p]
+        L.hepf_tth_host.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_int32, C.c_uint64,
+                                    C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                    C.c_size_t, C.c_void_p]
+        L.hepf_fp64_peak_probe.argtypes = [C.c_int, C.c_int, C.c_int64, C.c_void_p, C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def last_error() -> str:
+    return load().hepf_last_error().decode()
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise HepfError(f"{what} failed ({rc}): {last_error()}")
+
+
+def launch_count(reset: bool = False) -> int:
+    return int(load().hepf_launch_count(int(reset)))
+
+
+def default_params(**over) -> Params:
+    p = Params()
+    load().hepf_default_params(C.byref(p))
+    for k, v in over.items():
+        setattr(p, k, v)
+    return p
+
+
+def make_cuts(chain):
+    arr = (_Cut * max(1, len(chain)))()
+    for i, (kind, n, lo, hi) in enumerate(chain):
+        arr[i] = _Cut(int(kind), int(n), float(lo), float(hi))
+    return arr
+
+
+def _stream_ptr(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _view(base_ptr: int, flags_ptr: int, n_events: int, stride: int, event_base: int) -> _Events:
+    ev = _Events()
+    ev.n_events, ev.stride, ev.event_base = n_events, stride, event_base
+    for name, row in ROW.items():
+        setattr(ev, name, base_ptr + row * stride * 8)
+    ev.flags = flags_ptr
+    return ev
+
+
+class DeviceEvents:
+    """SoA event store resident in HBM: one [64, stride] float64 tensor + one [stride] int32 (uint32 bits) tensor."""
+
+    def __init__(self, cols, flags, n_events: int, event_base: int = 0):
+        assert cols.is_cuda and cols.dim() == 2 and cols.shape[0] == NROW and cols.is_contiguous()
+        self.cols, self.flags = cols, flags
+        self.n_events, self.stride, self.event_base = int(n_events), int(cols.shape[1]), int(event_base)
+
+    @classmethod
+    def from_host(cls, store, device="cuda", non_blocking: bool = False):
+        """Upload a host store (hepf_synth.EventStore or anything with cols/flags/n_events/event_base)."""
+        import torch
+        cols = torch.from_numpy(store.cols).to(device, non_blocking=non_blocking)
+        flags = torch.from_numpy(store.flags.view(np.int32)).to(device, non_blocking=non_blocking)
+        return cls(cols, flags, store.n_events, store.event_base)
+
+    def view(self) -> _Events:
+        return _view(self.cols.data_ptr(), self.flags.data_ptr(), self.n_events, self.stride, self.event_base)
+
+
+def select(events: DeviceEvents, chain, *, with_cutflow: bool = True, out_idx=None, out_count=None, out_cutflow=None,
+           ws=None, stream=None):
+    """hepf_select: returns (out_idx[int32 tensor, capacity n_events], out_count[int64 tensor(1)], cutflow or None).
+    Asynchronous on the stream; read ``out_count.item()`` (a sync) to learn how many entries of out_idx are valid."""
+    import torch
+    L = load()
+    dev = events.cols.device
+    n = events.n_events
+    if out_idx is None:
+        out_idx = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    if out_count is None:
+        out_count = torch.zeros(1, dtype=torch.int64, device=dev)
+    if with_cutflow and out_cutflow is None:
+        out_cutflow = torch.zeros(max(len(chain), 1), dtype=torch.int64, device=dev)
+    need = L.hepf_select_workspace_bytes(n)
+    if ws is None or ws.numel() < need:
+        ws = torch.empty(max(need, 16), dtype=torch.uint8, device=dev)
+    ev = events.view()
+    rc = L.hepf_select(C.byref(ev), make_cuts(chain), len(chain), out_idx.data_ptr(), out_count.data_ptr(),
+                       out_cutflow.data_ptr() if with_cutflow else None, ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc, "hepf_select")
+    return out_idx, out_count, (out_cutflow[: len(chain)] if with_cutflow else None)
+
+
+def reconstruct_tth(events: DeviceEvents, idx, n_idx: int, n_variations: int, seed: int, params: Params | None = None,
+                    *, out_best=None, stream=None):
+    """hepf_reconstruct_tth: returns a uint8 tensor [n_idx, 128] of hepf_best_t records (see BEST_DTYPE)."""
+    import torch
+    L = load()
+    if out_best is None:
+        out_best = torch.empty((max(n_idx, 1), 128), dtype=torch.uint8, device=events.cols.device)
+    ev = events.view()
+    rc = L.hepf_reconstruct_tth(C.byref(ev), idx.data_ptr(), n_idx, n_variations, seed,
+                                C.byref(params) if params is not None else None, out_best.data_ptr(), None, 0,
+                                _stream_ptr(stream))
+    _check(rc, "hepf_reconstruct_tth")
+    return out_best[:n_idx]
+
+
+def best_to_numpy(out_best) -> np.ndarray:
+    return out_best.cpu().numpy().reshape(-1).view(BEST_DTYPE)
+
+
+def philox_normal(seed: int, counter: int, n: int, *, out=None, device="cuda", stream=None):
+    """hepf_philox_normal: out[i] = Z[counter + i] (float64 tensor)."""
+    import torch
+    L = load()
+    if out is None:
+        out = torch.empty(n, dtype=torch.float64, device=device)
+    rc = L.hepf_philox_normal(seed, counter, n, out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "hepf_philox_normal")
+    return out
+
+
+def tth_host_arena_bytes(n_events: int, n_variations: int) -> int:
+    return int(load().hepf_tth_host_arena_bytes(n_events, n_variations))
+
+
+def tth_host(store, chain, n_variations: int, seed: int, params: Params | None = None, *, arena=None, out_best=None,
+             out_idx=None, stream=None):
+    """hepf_tth_host: whole path from HOST buffers (store.cols / store.flags are numpy arrays or pinned torch CPU
+    tensors).  Returns (idx[n_sel] uint32, best[n_sel] BEST_DTYPE, cutflow int64[n_cuts])."""
+    import torch
+    L = load()
+    n = store.n_events
+    cols_ptr = store.cols.data_ptr() if hasattr(store.cols, "data_ptr") else store.cols.ctypes.data
+    flags_ptr = store.flags.data_ptr() if hasattr(store.flags, "data_ptr") else store.flags.ctypes.data
+    ev = _view(cols_ptr, flags_ptr, n, store.stride, store.event_base)
+    need = L.hepf_tth_host_arena_bytes(n, n_variations)
+    if arena is None or arena.numel() < need:
+        arena = torch.empty(need, dtype=torch.uint8, device="cuda")
+    if out_best is None:
+        out_best = np.empty(max(n, 1), dtype=BEST_DTYPE)
+    if out_idx is None:
+        out_idx = np.empty(max(n, 1), dtype=np.uint32)
+    count = np.zeros(1, dtype=np.int64)
+    cutflow = np.zeros(max(len(chain), 1), dtype=np.int64)
+    ptr = lambda a: a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+    rc = L.hepf_tth_host(C.byref(ev), make_cuts(chain), len(chain), n_variations, seed,
+                         C.byref(params) if params is not None else None, ptr(out_idx), ptr(out_best),
+                         count.ctypes.data, cutflow.ctypes.data, arena.data_ptr(), arena.numel(), _stream_ptr(stream))
+    _check(rc, "hepf_tth_host")
+    n_sel = int(count[0])
+    return out_idx[:n_sel], out_best[:n_sel], cutflow[: len(chain)]
+
+
+def fp64_peak_probe(blocks: int, threads: int, fma_per_thread: int, sink, stream=None):
+    rc = load().hepf_fp64_peak_probe(blocks, threads, fma_per_thread, sink.data_ptr(), _stream_ptr(stream))
+    _check(rc, "hepf_fp64_peak_probe")

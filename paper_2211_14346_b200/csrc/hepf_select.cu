@@ -1,0 +1,248 @@
+// hepf_select.cu — hepf_select: ordered cut chain + stable stream compaction.
+//
+// Paper: a cut is `bool f(event)`, cuts are registered in order and an event is dropped at the first false
+// (PAPER.md:96-102, :286-295); the survivors are the filtered output.  §4 (:136): "eighteen
+// cuts, organised in a sequential way, as a computational pipeline".
+//
+// B200 mapping: the chain is HBM-bound (<= 180 B of columns per event, a handful of compares), so
+//   K1 select_eval   : one thread = two adjacent events, every needed column read with 128-bit loads that are
+//                      all issued before the first use (>= 20 independent 16-byte loads in flight per thread);
+//                      cuts evaluated from registers; __ballot_sync -> two 32-bit survivor masks per warp
+//                      (even/odd events) written to the workspace; per-block survivor count; cutflow by
+//                      ballot/popc + one atomicAdd per cut per block.
+//   K2 select_scatter: each block sums the counts of the blocks before it (<= 1184 values), then replays its
+//                      range from the 1-bit-per-event masks (1/1440 of K1's traffic) and writes the ascending
+//                      index list with popc-prefix offsets.  Deterministic, no atomics on the index cursor.
+// Each block owns a contiguous range of 512-event tiles; the grid is 8 blocks per SM (one wave).
+#include "hepf_common.cuh"
+
+namespace hepf {
+
+constexpr int SEL_THREADS = 256;
+constexpr int SEL_TILE = SEL_THREADS * 2;   // events per block iteration
+constexpr int SEL_WARPS = SEL_THREADS / 32;
+
+enum : uint32_t { NEED_LEP_PT = 1, NEED_LEP_ETA = 2, NEED_JET_PT = 4, NEED_JET_ETA = 8, NEED_MET = 16, NEED_MLL = 32 };
+
+struct CutChain {
+  int n;
+  uint32_t need;
+  hepf_cut_t c[HEPF_MAX_CUTS];
+};
+
+struct SelCols {
+  const double *lep_pt, *lep_eta, *jet_pt, *jet_eta, *met, *mll;
+  const uint32_t* flags;
+  int64_t n, stride;
+};
+
+__device__ __forceinline__ double2 ld2(const double* p) { return __ldcs(reinterpret_cast<const double2*>(p)); }
+__device__ __forceinline__ double pick(const double2& v, int k) { return k ? v.y : v.x; }
+
+__global__ void __launch_bounds__(SEL_THREADS)
+select_eval_kernel(SelCols ev, CutChain chain, int64_t n_tiles, int64_t tiles_per_block, uint2* __restrict__ masks,
+                   uint32_t* __restrict__ block_count, unsigned long long* __restrict__ cutflow) {
+  __shared__ unsigned int s_cf[HEPF_MAX_CUTS];
+  __shared__ unsigned int s_count;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid < HEPF_MAX_CUTS) s_cf[tid] = 0;
+  if (tid == 0) s_count = 0;
+  __syncthreads();
+  const int64_t t0 = (int64_t)blockIdx.x * tiles_per_block;
+  const int64_t t1 = min(t0 + tiles_per_block, n_tiles);
+  unsigned int my_cf = 0, my_count = 0;   // lane c accumulates cut c; lane 0 accumulates survivors
+  for (int64_t t = t0; t < t1; t++) {
+    const int64_t i0 = t * SEL_TILE + 2 * tid;            // first of this thread's two events
+    bool pass[2] = {false, false};
+    int fail_at[2] = {0, 0};                              // number of cuts passed
+    if (i0 < ev.n) {                                      // i0 + 1 <= stride - 1 is always readable (stride even)
+      const uint2 fl = __ldcs(reinterpret_cast<const uint2*>(ev.flags + i0));
+      double2 lpt[2], leta[2], jpt[HEPF_N_JET], jeta[HEPF_N_JET], met, mll;
+      // ---- issue every load the chain needs before any use -----------------------------------------------
+      if (chain.need & NEED_LEP_PT) { lpt[0] = ld2(ev.lep_pt + i0); lpt[1] = ld2(ev.lep_pt + ev.stride + i0); }
+      if (chain.need & NEED_LEP_ETA) { leta[0] = ld2(ev.lep_eta + i0); leta[1] = ld2(ev.lep_eta + ev.stride + i0); }
+      if (chain.need & NEED_JET_PT) {
+#pragma unroll
+        for (int s = 0; s < HEPF_N_JET; s++) jpt[s] = ld2(ev.jet_pt + s * ev.stride + i0);
+      }
+      if (chain.need & NEED_JET_ETA) {
+#pragma unroll
+        for (int s = 0; s < HEPF_N_JET; s++) jeta[s] = ld2(ev.jet_eta + s * ev.stride + i0);
+      }
+      if (chain.need & NEED_MET) met = ld2(ev.met + i0);
+      if (chain.need & NEED_MLL) mll = ld2(ev.mll + i0);
+      // ---- evaluate the chain from registers ------------------------------------------------------------------
+#pragma unroll
+      for (int k = 0; k < 2; k++) {
+        const uint32_t f = k ? fl.y : fl.x;
+        const int n_lep = f & 15u, n_jet = min(8u, (f >> 8) & 15u);
+        bool alive = (i0 + k) < ev.n;
+        int passed = 0;
+        for (int c = 0; c < chain.n && alive; c++) {
+          const hepf_cut_t cut = chain.c[c];
+          bool ok = false;
+          switch (cut.kind) {
+            case HEPF_CUT_NLEP_EQ: ok = n_lep == (int)cut.n; break;
+            case HEPF_CUT_LEP_OS: ok = ((f >> 4) & 1u) != ((f >> 5) & 1u); break;
+            case HEPF_CUT_LEP_PT_GT: ok = pick(lpt[0], k) > cut.lo && pick(lpt[1], k) > cut.lo; break;
+            case HEPF_CUT_LEP_ABSETA_LT: ok = fabs(pick(leta[0], k)) < cut.hi && fabs(pick(leta[1], k)) < cut.hi; break;
+            case HEPF_CUT_NJET_GE:
+            case HEPF_CUT_NBJET_GE: {
+              const uint32_t tagmask = cut.kind == HEPF_CUT_NBJET_GE ? (f >> 16) : 0xffu;
+              int cnt = 0;
+#pragma unroll
+              for (int s = 0; s < HEPF_N_JET; s++)
+                cnt += (s < n_jet) && ((tagmask >> s) & 1u) && pick(jpt[s], k) > cut.lo && fabs(pick(jeta[s], k)) < cut.hi;
+              ok = cnt >= (int)cut.n;
+            } break;
+            case HEPF_CUT_MET_GT: ok = pick(met, k) > cut.lo; break;
+            case HEPF_CUT_MLL_GT: ok = pick(mll, k) > cut.lo; break;
+            case HEPF_CUT_MLL_OUTSIDE: ok = pick(mll, k) < cut.lo || pick(mll, k) > cut.hi; break;
+            default: ok = false;
+          }
+          alive = ok;
+          passed += ok;
+        }
+        pass[k] = alive;
+        fail_at[k] = passed;
+      }
+    }
+    // ---- warp compaction: survivor masks (even events, odd events) ---------------------------------------------
+    const unsigned b0 = __ballot_sync(0xffffffffu, pass[0]), b1 = __ballot_sync(0xffffffffu, pass[1]);
+    if (lane == 0) {
+      masks[t * SEL_WARPS + warp] = make_uint2(b0, b1);
+      my_count += __popc(b0) + __popc(b1);
+    }
+    if (cutflow) {
+      for (int c = 0; c < chain.n; c++) {
+        const unsigned m0 = __ballot_sync(0xffffffffu, fail_at[0] > c), m1 = __ballot_sync(0xffffffffu, fail_at[1] > c);
+        if (lane == c) my_cf += __popc(m0) + __popc(m1);
+      }
+    }
+  }
+  if (lane == 0 && my_count) atomicAdd(&s_count, my_count);
+  if (cutflow && lane < chain.n && my_cf) atomicAdd(&s_cf[lane], my_cf);
+  __syncthreads();
+  if (tid == 0) block_count[blockIdx.x] = s_count;
+  if (cutflow && tid < chain.n && s_cf[tid]) atomicAdd(&cutflow[tid], (unsigned long long)s_cf[tid]);
+}
+
+__global__ void __launch_bounds__(SEL_THREADS)
+select_scatter_kernel(int64_t n_tiles, int64_t tiles_per_block, const uint2* __restrict__ masks,
+                      const uint32_t* __restrict__ block_count, uint32_t* __restrict__ out_idx,
+                      int64_t* __restrict__ out_count) {
+  __shared__ unsigned long long s_part[SEL_WARPS];
+  __shared__ unsigned int s_wcount[SEL_WARPS];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  // exclusive offset of this block = sum of the counts of the blocks before it (grid <= ~1.2k blocks)
+  unsigned long long part = 0;
+  const int upto = (blockIdx.x == 0) ? gridDim.x : blockIdx.x;   // block 0 also produces the grand total
+  for (int b = tid; b < upto; b += SEL_THREADS) part += block_count[b];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+  if (lane == 0) s_part[warp] = part;
+  __syncthreads();
+  unsigned long long base = 0;
+#pragma unroll
+  for (int w = 0; w < SEL_WARPS; w++) base += s_part[w];
+  if (blockIdx.x == 0) {
+    if (tid == 0) *out_count = (int64_t)base;
+    base = 0;
+  }
+  const int64_t t0 = (int64_t)blockIdx.x * tiles_per_block;
+  const int64_t t1 = min(t0 + tiles_per_block, n_tiles);
+  for (int64_t t = t0; t < t1; t++) {
+    const uint2 m = masks[t * SEL_WARPS + warp];
+    const unsigned wc = __popc(m.x) + __popc(m.y);
+    __syncthreads();                      // s_wcount of the previous tile fully consumed
+    if (lane == 0) s_wcount[warp] = wc;
+    __syncthreads();
+    unsigned before = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < SEL_WARPS; w++) { const unsigned c = s_wcount[w]; before += (w < warp) ? c : 0; total += c; }
+    const unsigned lt = (1u << lane) - 1u;
+    const unsigned p0 = (m.x >> lane) & 1u, p1 = (m.y >> lane) & 1u;
+    const unsigned long long pos = base + before + __popc(m.x & lt) + __popc(m.y & lt);
+    const int64_t i0 = t * SEL_TILE + 2 * tid;
+    if (p0) out_idx[pos] = (uint32_t)i0;
+    if (p1) out_idx[pos + p0] = (uint32_t)(i0 + 1);
+    base += total;
+  }
+}
+
+}  // namespace hepf
+
+using namespace hepf;
+
+static void sel_geometry(int64_t n_events, int sms, int64_t* n_tiles, int* grid, int64_t* tiles_per_block) {
+  *n_tiles = (n_events + SEL_TILE - 1) / SEL_TILE;
+  int64_t g = *n_tiles < (int64_t)sms * 8 ? *n_tiles : (int64_t)sms * 8;
+  if (g < 1) g = 1;
+  *tiles_per_block = (*n_tiles + g - 1) / g;
+  if (*tiles_per_block < 1) *tiles_per_block = 1;
+  *grid = (int)((*n_tiles + *tiles_per_block - 1) / *tiles_per_block);
+  if (*grid < 1) *grid = 1;
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+extern "C" size_t hepf_select_workspace_bytes(int64_t n_events) {
+  if (n_events < 0) return 0;
+  const int64_t n_tiles = (n_events + SEL_TILE - 1) / SEL_TILE;
+  // masks: one uint2 per warp-tile; block counts: at most 8 blocks per SM, sized generously for 4096 blocks
+  return align_up((size_t)(n_tiles + 1) * SEL_WARPS * sizeof(uint2), 256) + 4096 * sizeof(uint32_t);
+}
+
+extern "C" int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
+                           int64_t* out_count, int64_t* out_cutflow, void* ws, size_t ws_bytes, void* stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  int rc = check_events(events);
+  if (rc != HEPF_OK) return rc;
+  if (n_cuts < 0 || n_cuts > HEPF_MAX_CUTS || (n_cuts > 0 && !host_cuts)) {
+    set_error("hepf_select: n_cuts must be 0..%d with a non-NULL chain", HEPF_MAX_CUTS); return HEPF_ERR_ARG;
+  }
+  if (!out_count || !aligned(out_count, 8) || (events->n_events > 0 && (!out_idx || !aligned(out_idx, 4)))) {
+    set_error("hepf_select: output pointer NULL or misaligned"); return HEPF_ERR_ARG;
+  }
+  if (out_cutflow && !aligned(out_cutflow, 8)) { set_error("hepf_select: out_cutflow misaligned"); return HEPF_ERR_ARG; }
+  const int64_t n = events->n_events;
+  if (ws_bytes < hepf_select_workspace_bytes(n) || !ws || !aligned(ws, 16)) {
+    set_error("hepf_select: workspace too small or misaligned (%zu < %zu)", ws_bytes, hepf_select_workspace_bytes(n));
+    return HEPF_ERR_CAPACITY;
+  }
+  CutChain chain{};
+  chain.n = n_cuts;
+  for (int c = 0; c < n_cuts; c++) {
+    chain.c[c] = host_cuts[c];
+    switch (host_cuts[c].kind) {
+      case HEPF_CUT_LEP_PT_GT: chain.need |= NEED_LEP_PT; break;
+      case HEPF_CUT_LEP_ABSETA_LT: chain.need |= NEED_LEP_ETA; break;
+      case HEPF_CUT_NJET_GE: case HEPF_CUT_NBJET_GE: chain.need |= NEED_JET_PT | NEED_JET_ETA; break;
+      case HEPF_CUT_MET_GT: chain.need |= NEED_MET; break;
+      case HEPF_CUT_MLL_GT: case HEPF_CUT_MLL_OUTSIDE: chain.need |= NEED_MLL; break;
+      case HEPF_CUT_NLEP_EQ: case HEPF_CUT_LEP_OS: break;
+      default: set_error("hepf_select: unknown cut kind %u at position %d", host_cuts[c].kind, c); return HEPF_ERR_ARG;
+    }
+  }
+  if (out_cutflow && n_cuts > 0) HEPF_CUDA_TRY(cudaMemsetAsync(out_cutflow, 0, sizeof(int64_t) * n_cuts, stream));
+  if (n == 0) { HEPF_CUDA_TRY(cudaMemsetAsync(out_count, 0, sizeof(int64_t), stream)); return HEPF_OK; }
+  int dev = 0, sms = 148;
+  HEPF_CUDA_TRY(cudaGetDevice(&dev));
+  HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  int64_t n_tiles, tpb; int grid;
+  sel_geometry(n, sms, &n_tiles, &grid, &tpb);
+  if (grid > 4096) { set_error("hepf_select: grid %d exceeds the workspace layout", grid); return HEPF_ERR_CAPACITY; }
+  uint2* masks = reinterpret_cast<uint2*>(ws);
+  uint32_t* block_count = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(ws) +
+                                                      align_up((size_t)(n_tiles + 1) * SEL_WARPS * sizeof(uint2), 256));
+  SelCols cols{events->lep_pt, events->lep_eta, events->jet_pt, events->jet_eta, events->met, events->mll,
+               events->flags, n, events->stride};
+  select_eval_kernel<<<grid, SEL_THREADS, 0, stream>>>(cols, chain, n_tiles, tpb, masks, block_count,
+                                                       (n_cuts > 0) ? reinterpret_cast<unsigned long long*>(out_cutflow) : nullptr);
+  count_launch();
+  HEPF_CUDA_TRY(cudaGetLastError());
+  select_scatter_kernel<<<grid, SEL_THREADS, 0, stream>>>(n_tiles, tpb, masks, block_count, out_idx, out_count);
+  count_launch();
+  HEPF_CUDA_TRY(cudaGetLastError());
+  return HEPF_OK;
+}

@@ -1,0 +1,123 @@
+"""GPU-vs-oracle comparison of hepf_best_t records with the conditioning-aware rules of DESIGN.md R11.
+
+north_star: chosen indices bit-exact "except where the oracle's top two likelihoods differ by < 1e-9 relative";
+masses and momenta within 1e-9 relative in FP64.  The solve is ill-conditioned near tangent conics, so the
+per-event tolerance is max(1e-9, 64 kappa) with kappa = eps sum|h_i x^i| / |x P'(x)| reported by the oracle, and an
+index mismatch is excused only in the classes below; everything else fails.
+"""
+from __future__ import annotations
+
+import math
+from collections import Counter
+
+import numpy as np
+
+import oracle
+
+IDX_KEYS = ("variation", "jet_b", "jet_bbar", "jet_h1", "jet_h2", "root")
+TANGENT = 1e-11     # |P| / sum|h_i x^i| at a critical point below this = near-tangent conics (class iii)
+
+
+def _cands(flags: int):
+    n_jet = min(8, (flags >> 8) & 15)
+    return [s for s in range(n_jet) if (flags >> (16 + s)) & 1][:6]
+
+
+def _cell_of(store, rec):
+    c = _cands(int(store.flags[rec["event"]]))
+    nb = len(c)
+    i, j = c.index(int(rec["jet_b"])), c.index(int(rec["jet_bbar"]))
+    rest = [(k, l) for k in range(nb) for l in range(k + 1, nb) if not {k, l} & {i, j}]
+    h = rest.index((c.index(int(rec["jet_h1"])), c.index(int(rec["jet_h2"]))))
+    return i * nb + j, h
+
+
+def _close(a, b, tol, scale=None):
+    a, b = np.asarray(a, float), np.asarray(b, float)
+    s = max(np.abs(b).max(), 1.0) if scale is None else scale
+    return bool(np.all(np.abs(a - b) <= tol * s))
+
+
+def compare(store, gpu, orc, aux, n_variations, seed, params=None, m_top=172.5, m_w=80.4):
+    """Returns (Counter of classes, list of failure strings)."""
+    cls, fails = Counter(), []
+    for k in range(len(orc)):
+        g, o, ax = gpu[k], orc[k], aux[k]
+        e = int(o["event"])
+        if int(g["event"]) != e:
+            fails.append(f"k={k}: event {g['event']} != {e}"); continue
+        if (int(g["status"]) & 6) != (int(o["status"]) & 6):
+            fails.append(f"e={e}: applicability/truncation bits {g['status']} != {o['status']}"); continue
+        gs, os_ = int(g["status"]) & 1, int(o["status"]) & 1
+        kap = float(ax["kappa"]) if np.isfinite(ax["kappa"]) else 0.0
+        tol = max(1e-9, 64 * kap)
+        if not gs and not os_:
+            ok = all(np.isnan(g[f]).all() for f in ("nu", "nubar", "loglik", "m_top")) and all(g[f] == -1 for f in IDX_KEYS)
+            cls["both_unsolved"] += 1
+            if not ok:
+                fails.append(f"e={e}: unsolved record is not NaN/-1")
+            continue
+        if gs and os_ and all(int(g[f]) == int(o[f]) for f in IDX_KEYS):
+            pscale = max(np.abs(o["nu"]).max(), np.abs(o["nubar"]).max())
+            ok = (_close(g["nu"], o["nu"], tol, pscale) and _close(g["nubar"], o["nubar"], tol, pscale)
+                  and _close(g["loglik"], o["loglik"], tol, max(1.0, abs(o["loglik"])))
+                  and all(_close(g[f], o[f], tol, o[f]) for f in ("m_top", "m_antitop", "m_wplus", "m_wminus", "m_higgs")))
+            # closure of the GPU record itself: the imposed masses come back
+            ok_closure = all(abs(g[f] - m) <= 10 * tol * m for f, m in (("m_top", m_top), ("m_antitop", m_top),
+                                                                        ("m_wplus", m_w), ("m_wminus", m_w)))
+            cls["match" if tol == 1e-9 else "match_kappa_tol"] += 1
+            if not ok:
+                fails.append(f"e={e}: same indices, values differ beyond tol={tol:.2e} "
+                             f"(nu {g['nu']} vs {o['nu']}, ll {g['loglik']!r} vs {o['loglik']!r})")
+            elif not ok_closure:
+                fails.append(f"e={e}: closure violated m_t={g['m_top']} m_W={g['m_wplus']}")
+            continue
+        # ---- index or status mismatch: classify -------------------------------------------------------------------
+        why = None
+        best_o = float(o["loglik"]) if os_ else -math.inf
+        if gs:
+            a_g, h_g = _cell_of(store, g)
+            P = oracle.eval_cell(store, e, int(g["variation"]), a_g, seed, params)
+            near = None
+            for r in range(P.n_roots):
+                if abs(P.x[r] - g["nu"][0]) <= max(1e-7, 1e3 * P.kappa[r]) * max(1.0, abs(P.x[r])):
+                    near = r
+            if near is not None:
+                ll = P.hterm[h_g] + P.nterm[near]
+                if os_ and abs(ll - best_o) <= 1e-9 * max(1.0, abs(best_o)):
+                    why = "tie_equivalent_candidate"           # (i)/(ii): same likelihood up to 1e-9
+                elif os_ and abs(best_o - float(ax["loglik2"])) <= 1e-9 * max(1.0, abs(best_o)):
+                    why = "tie_top_two"
+                elif os_ and ll > best_o:
+                    why = None                                 # oracle itself prefers it?  impossible -> fail
+            else:
+                if P.min_abs_p_rel < TANGENT:                  # (iii): GPU resolved a tangency the bisection skipped
+                    closure = all(abs(g[f] - m) <= 1e-6 * m for f, m in (("m_top", m_top), ("m_antitop", m_top),
+                                                                         ("m_wplus", m_w), ("m_wminus", m_w)))
+                    if closure:
+                        why = "tangent_root_gpu_only"
+        if why is None and os_:
+            # did the GPU miss the oracle's winning root because it sits at a near-tangency?
+            a_o, _ = int(ax["pairing"]), int(ax["higgs_pair"])
+            P = oracle.eval_cell(store, e, int(o["variation"]), a_o, seed, params)
+            if P.min_abs_p_rel < TANGENT or kap > 1e-9:
+                why = "tangent_root_oracle_only"
+        if why is None:
+            fails.append(f"e={e}: UNEXCUSED mismatch gpu(status={g['status']}, v={g['variation']}, b={g['jet_b']}, "
+                         f"bbar={g['jet_bbar']}, root={g['root']}, ll={g['loglik']!r}) vs oracle(status={o['status']}, "
+                         f"v={o['variation']}, b={o['jet_b']}, bbar={o['jet_bbar']}, root={o['root']}, ll={o['loglik']!r}, "
+                         f"ll2={ax['loglik2']!r}, kappa={kap:.2e})")
+        else:
+            cls[why] += 1
+    return cls, fails
+
+
+def assert_parity(store, gpu, orc, aux, n_variations, seed, params=None, max_excused_frac=2e-3, label=""):
+    cls, fails = compare(store, gpu, orc, aux, n_variations, seed, params)
+    n = len(orc)
+    exact = cls["match"] + cls["match_kappa_tol"] + cls["both_unsolved"]
+    excused = n - exact - len(fails)
+    print(f"[parity {label}] n={n} classes={dict(cls)} failures={len(fails)}")
+    assert not fails, "\n".join(fails[:10])
+    assert excused <= max(2, max_excused_frac * n), (excused, n, dict(cls))
+    return cls

@@ -1,0 +1,253 @@
+"""-m gpu: the CUDA path (through the C ABI binding) against the oracle, element by element."""
+import numpy as np
+import pytest
+
+import hepf_synth as hs
+import oracle
+from parity import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def hepf():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2211_14346_b200 as h
+    h.load()
+    return h
+
+
+def _gpu_select(hepf, store, chain):
+    import torch
+    dev = hepf.DeviceEvents.from_host(store)
+    idx, count, cf = hepf.select(dev, chain)
+    torch.cuda.synchronize()
+    n = int(count.item())
+    return dev, idx, n, idx[:n].cpu().numpy().view(np.uint32), cf.cpu().numpy()
+
+
+def _gpu_reco(hepf, dev, idx_t, n, V, seed, params=None):
+    import torch
+    from paper_2211_14346_b200.binding import best_to_numpy
+    out = hepf.reconstruct_tth(dev, idx_t, n, V, seed, params)
+    torch.cuda.synchronize()
+    return best_to_numpy(out)
+
+
+# ------------------------------------------------------------------------------------------------ philox / normals
+def test_philox_normal_prefix_bit_exact(hepf):
+    import torch
+    n = 1 << 20
+    got = hepf.philox_normal(7, 0, n).cpu().numpy()
+    want = oracle.philox_normal(7, 0, n)
+    assert got.tobytes() == want.tobytes()
+
+
+@pytest.mark.parametrize("counter,n,offset", [(0, 1, 0), (1, 1, 0), (1, 2, 0), (3, 1001, 0), (0, 777, 1), (5, 4096, 1),
+                                              ((1 << 35) + 3, 5000, 0), ((1 << 33), 4097, 1), (2, 0, 0)])
+def test_philox_normal_ragged_ranges_and_alignment(hepf, counter, n, offset):
+    import torch
+    buf = torch.full((n + 4,), -7.0, dtype=torch.float64, device="cuda")
+    hepf.philox_normal(11, counter, n, out=buf[offset:offset + n] if n else buf[0:0])
+    torch.cuda.synchronize()
+    got = buf.cpu().numpy()
+    want = oracle.philox_normal(11, counter, n)
+    assert got[offset:offset + n].tobytes() == want.tobytes()
+    assert (got[:offset] == -7.0).all() and (got[offset + n:] == -7.0).all()     # nothing written outside
+
+
+def test_philox_normal_split_invariance(hepf):
+    import torch
+    a = hepf.philox_normal(7, 10, 100_003).cpu().numpy()
+    b = np.concatenate([hepf.philox_normal(7, 10, 50_001).cpu().numpy(), hepf.philox_normal(7, 50_011, 50_002).cpu().numpy()])
+    assert a.tobytes() == b.tobytes()
+
+
+# ------------------------------------------------------------------------------------------------------------ select
+@pytest.mark.parametrize("cfg_id,n", [(1, 10_000), (4, 1_000_000), (3, 100_000)])
+def test_select_matches_oracle_exactly(hepf, cfg_id, n):
+    cfg = hs.CONFIGS[cfg_id]
+    st = cfg.events(n)
+    want_idx, want_cf = oracle.select(st, cfg.cuts)
+    _, _, n_sel, got_idx, got_cf = _gpu_select(hepf, st, cfg.cuts)
+    assert n_sel == len(want_idx)
+    assert np.array_equal(got_idx, want_idx)
+    assert np.array_equal(got_cf, want_cf)
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 63, 64, 511, 512, 513, 1025, 40_001])
+def test_select_ragged_sizes_and_empty_chain(hepf, n):
+    st = hs.generate(max(n, 1), 9, bkg_frac=0.3, with_truth=False)
+    st.n_events = n
+    for chain in (hs.CHAIN_TIGHT8[:5], hs.CHAIN_BASE, []):
+        want_idx, want_cf = oracle.select(st, chain)
+        _, _, n_sel, got_idx, got_cf = _gpu_select(hepf, st, chain)
+        assert n_sel == len(want_idx) and np.array_equal(got_idx, want_idx)
+        assert np.array_equal(got_cf[: len(chain)], want_cf)
+
+
+def test_select_every_cut_kind_with_thresholds_and_nan(hepf):
+    st = hs.generate(50_000, 10, bkg_frac=0.5, with_truth=False)
+    rng = np.random.default_rng(0)
+    # plant exact-threshold values and NaNs
+    st.cols[hs.ROW["met"], :1000] = 30.0
+    st.cols[hs.ROW["mll"], 1000:2000] = 40.0
+    st.cols[hs.ROW["met"], 2000:2100] = np.nan
+    st.cols[hs.ROW["lep_pt"], 2100:2200] = np.nan
+    st.cols[hs.ROW["jet_eta"] + 1, 3000:4000] = -2.5
+    st.cols[hs.ROW["jet_pt"] + 2, 4000:5000] = 25.0
+    chains = [
+        [(hs.MET_GT, 0, 30.0, 0)], [(hs.MLL_GT, 0, 40.0, 0)], [(hs.MLL_OUTSIDE, 0, 80.0, 100.0)],
+        [(hs.LEP_PT_GT, 0, 25.0, 0)], [(hs.LEP_ABSETA_LT, 0, 0, 1.5)], [(hs.NJET_GE, 3, 25.0, 2.5)],
+        [(hs.NBJET_GE, 2, 30.0, 2.0)], [(hs.NLEP_EQ, 3, 0, 0)], [(hs.LEP_OS, 0, 0, 0)],
+        [(hs.NJET_GE, 0, 1e9, 2.5)], [(hs.NJET_GE, 9, 0.0, hs.INF)],
+        hs.CHAIN_TIGHT8 + [(hs.MLL_OUTSIDE, 0, 81.0, 101.0), (hs.NBJET_GE, 4, 45.0, 2.4)],
+    ]
+    for chain in chains:
+        want_idx, want_cf = oracle.select(st, chain)
+        _, _, n_sel, got_idx, got_cf = _gpu_select(hepf, st, chain)
+        assert np.array_equal(got_idx, want_idx), chain
+        assert np.array_equal(got_cf, want_cf), chain
+
+
+def test_select_rejects_bad_arguments(hepf):
+    st = hs.generate(10, 1, with_truth=False)
+    dev = hepf.DeviceEvents.from_host(st)
+    with pytest.raises(hepf.HepfError):
+        hepf.select(dev, [(99, 0, 0, 0)])
+    with pytest.raises(hepf.HepfError):
+        hepf.select(dev, [(hs.MET_GT, 0, 1.0, 0)] * 33)
+
+
+# ------------------------------------------------------------------------------------------------------ reconstruct
+def test_cfg1_full_parity(hepf):
+    cfg = hs.CONFIGS[1]
+    st = cfg.events()
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, cfg.cuts)
+    got = _gpu_reco(hepf, dev, idx_t, n, cfg.n_variations, cfg.reco_seed)
+    want, aux = oracle.reconstruct_tth(st, idx, cfg.n_variations, cfg.reco_seed, n_threads=8)
+    cls = assert_parity(st, got, want, aux, cfg.n_variations, cfg.reco_seed, label="cfg1")
+    assert cls["match"] > 0.9 * len(idx)
+
+
+@pytest.mark.parametrize("V", [1, 3, 16, 33, 48, 64, 130, 256])
+def test_variation_counts_and_lane_mappings(hepf, V):
+    st = hs.generate(600, 21, with_truth=False)
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, hs.CHAIN_BASE)
+    m = min(n, 64 if V > 64 else 200)
+    got = _gpu_reco(hepf, dev, idx_t, m, V, 1234 + V)
+    want, aux = oracle.reconstruct_tth(st, idx[:m], V, 1234 + V, n_threads=8)
+    assert_parity(st, got, want, aux, V, 1234 + V, label=f"V={V}")
+
+
+def test_six_b_candidates_parity(hepf):
+    cfg = hs.CONFIGS[3]
+    st = cfg.events(3000)
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, cfg.cuts)
+    m = min(n, 300)
+    got = _gpu_reco(hepf, dev, idx_t, m, 32, cfg.reco_seed)
+    want, aux = oracle.reconstruct_tth(st, idx[:m], 32, cfg.reco_seed, n_threads=8)
+    assert_parity(st, got, want, aux, 32, cfg.reco_seed, label="cfg3-sample")
+    assert (got["jet_h1"] >= 0).sum() > 0.8 * m
+
+
+def test_background_topologies_status_bits(hepf):
+    st = hs.generate(20_000, 8, bkg_frac=1.0, with_truth=False)
+    dev = hepf.DeviceEvents.from_host(st)
+    import torch
+    idx = np.arange(st.n_events, dtype=np.uint32)
+    idx_t = torch.from_numpy(idx.view(np.int32)).cuda()
+    got = _gpu_reco(hepf, dev, idx_t, len(idx), 4, 77)
+    sel = np.nonzero((got["status"] & 2) == 0)[0]
+    want, aux = oracle.reconstruct_tth(st, idx, 4, 77, n_threads=8)
+    assert np.array_equal(got["status"] & 6, want["status"] & 6)
+    assert (got["status"] & 4).any() and (got["status"] & 2).any() and len(sel) > 20
+    assert_parity(st, got, want, aux, 4, 77, label="background")
+
+
+def test_sigma_scale_zero_picks_variation_zero(hepf):
+    st = hs.generate(2000, 5, with_truth=False)
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, hs.CHAIN_BASE)
+    P0 = hepf.default_params(sigma_scale=0.0)
+    g1 = _gpu_reco(hepf, dev, idx_t, n, 1, 5, P0)
+    g40 = _gpu_reco(hepf, dev, idx_t, n, 40, 5, P0)
+    assert g1.tobytes() == g40.tobytes()
+    want, aux = oracle.reconstruct_tth(st, idx, 1, 5, oracle.default_params(sigma_scale=0.0), n_threads=8)
+    assert_parity(st, g1, want, aux, 1, 5, oracle.default_params(sigma_scale=0.0), label="nominal")
+
+
+def test_event_base_split_invariance_and_prefix_property(hepf):
+    """Results depend on (seed, global event index, variation) only: not on the view split, not on the launch shape."""
+    st = hs.generate(3000, 6, with_truth=False)
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, hs.CHAIN_BASE)
+    whole = _gpu_reco(hepf, dev, idx_t, n, 24, 99)
+    cut = 1501
+    parts = []
+    for lo, hi in ((0, cut), (cut, st.n_events)):
+        sub = st.slice(lo, hi)
+        d2, i2, n2, _, _ = _gpu_select(hepf, sub, hs.CHAIN_BASE)
+        r = _gpu_reco(hepf, d2, i2, n2, 24, 99).copy()
+        r["event"] += lo
+        parts.append(r)
+    both = np.concatenate(parts)
+    assert both.tobytes() == whole.tobytes()
+    # prefix property in V
+    v64 = _gpu_reco(hepf, dev, idx_t, n, 64, 99)
+    keep = ((v64["status"] & 1) == 1) & (v64["variation"] < 24)
+    assert whole[keep].tobytes() == v64[keep].tobytes()
+    s = (whole["status"] & 1) == 1
+    assert (v64["loglik"][s] >= whole["loglik"][s]).all()
+
+
+def test_params_other_than_default(hepf):
+    st = hs.generate(800, 12, with_truth=False)
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, hs.CHAIN_BASE)
+    kw = dict(m_top=173.0, m_w=80.0, m_higgs=120.0, sigma_higgs=10.0, lambda_nu=55.0, lep_sigma=0.02, jet_stoch=0.8,
+              jet_const=0.05, sigma_scale=1.5, s_min=0.2)
+    got = _gpu_reco(hepf, dev, idx_t, n, 8, 3, hepf.default_params(**kw))
+    Po = oracle.default_params(**kw)
+    want, aux = oracle.reconstruct_tth(st, idx, 8, 3, Po, n_threads=8)
+    cls, fails = __import__("parity").compare(st, got, want, aux, 8, 3, Po, m_top=173.0, m_w=80.0)
+    assert not fails, fails[:5]
+
+
+def test_tth_host_equals_device_path(hepf):
+    cfg = hs.CONFIGS[1]
+    st = cfg.events(4001)
+    dev, idx_t, n, idx, cf = _gpu_select(hepf, st, cfg.cuts)
+    want = _gpu_reco(hepf, dev, idx_t, n, 8, 42)
+    hidx, hbest, hcf = hepf.tth_host(st, cfg.cuts, 8, 42)
+    assert np.array_equal(hidx, idx) and np.array_equal(hcf, cf)
+    assert hbest.tobytes() == want.tobytes()
+
+
+def test_reconstruct_rejects_bad_arguments(hepf):
+    st = hs.generate(10, 1, with_truth=False)
+    dev, idx_t, n, _, _ = _gpu_select(hepf, st, [])
+    with pytest.raises(hepf.HepfError):
+        hepf.reconstruct_tth(dev, idx_t, n, 0, 1)
+    with pytest.raises(hepf.HepfError):
+        hepf.reconstruct_tth(dev, idx_t, -1, 4, 1)
+
+
+# ------------------------------------------------------------------------------------- bench-size, sampled parity
+def test_cfg2_full_size_sampled_parity(hepf):
+    """BASELINE.json configs[1] at full size in the launch configuration bench.py times; the oracle checks every
+    selected event's selection exactly and a 1-in-400 sample of the reconstructed records."""
+    import torch
+    cfg = hs.CONFIGS[2]
+    st = cfg.events()
+    want_idx, want_cf = oracle.select(st, cfg.cuts)
+    dev, idx_t, n, idx, cf = _gpu_select(hepf, st, cfg.cuts)
+    assert np.array_equal(idx, want_idx) and np.array_equal(cf, want_cf)
+    got = _gpu_reco(hepf, dev, idx_t, n, cfg.n_variations, cfg.reco_seed)
+    assert np.array_equal(got["event"], idx)
+    solved = (got["status"] & 1) == 1
+    assert solved.mean() > 0.9
+    # property that holds at any size: closure of every reported solution
+    for f, m in (("m_top", 172.5), ("m_antitop", 172.5), ("m_wplus", 80.4), ("m_wminus", 80.4)):
+        assert np.nanmax(np.abs(got[f][solved] - m) / m) < 1e-6
+    sample = np.arange(0, n, 400)
+    want, aux = oracle.reconstruct_tth(st, idx[sample], cfg.n_variations, cfg.reco_seed, n_threads=8)
+    assert_parity(st, got[sample], want, aux, cfg.n_variations, cfg.reco_seed, label="cfg2-sampled")
