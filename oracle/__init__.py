@@ -46,8 +46,8 @@ BEST_DTYPE = np.dtype([("nu", "f8", 3), ("nubar", "f8", 3), ("m_top", "f8"), ("m
                        ("variation", "i4"), ("jet_b", "i4"), ("jet_bbar", "i4"), ("jet_h1", "i4"),
                        ("jet_h2", "i4"), ("root", "i4"), ("status", "u4"), ("event", "u4")])
 AUX_DTYPE = np.dtype([("kappa", "f8"), ("loglik2", "f8"), ("n_cand", "i8"), ("pairing", "i4"),
-                      ("higgs_pair", "i4")])
-assert BEST_DTYPE.itemsize == 128 and AUX_DTYPE.itemsize == 32
+                      ("higgs_pair", "i4"), ("pz_terms", "f8"), ("pzbar_terms", "f8")])
+assert BEST_DTYPE.itemsize == 128 and AUX_DTYPE.itemsize == 48
 
 
 class Pairing(C.Structure):

@@ -61,6 +61,7 @@ typedef struct {      /* per-event diagnostics the parity harness needs (DESIGN.
   double loglik2;     /* best log-likelihood among all other candidates (-inf if none)  */
   int64_t n_cand;     /* candidates enumerated                                          */
   int32_t pairing, higgs_pair; /* a = i*n_b + j and h of the winner                     */
+  double pz_terms, pzbar_terms; /* |c0|+|c1 x|+|c2 y| of the two p_z linear forms (R11b)  */
 } orc_aux_t;
 
 typedef struct {      /* one pairing solved in isolation (worked example, brute-force pins, R11 ii/iii) */

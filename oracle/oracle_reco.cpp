@@ -159,7 +159,7 @@ int quartic_roots(const double g[4], double roots[4]) {
 
 struct PairingSolution {
   int n_roots = 0;
-  double x[4], y[4], kappa[4], nterm[4];
+  double x[4], y[4], kappa[4], nterm[4], sz[4], szb[4];   // sz: sum of |terms| of the p_z linear forms (R11b)
   V4 nu[4], nub[4];
   Resultant R; double g[4]; Conic k1, k2; double min_abs_p_rel = 1.0;
 };
@@ -209,10 +209,24 @@ PairingSolution solve_pairing(const V4& lp, const V4& b, const V4& lm, const V4&
       };
       y = res2(y1) <= res2(y2) ? y1 : y2;
     }
+    // Two Newton steps on the pair of conics in (x, y) — the defining equations of the intersection.  The
+    // quotient -D1/D2 cancels catastrophically when D2(x) is small, and north_star asks for 1e-9 (R11a).
+    for (int it = 0; it < 2; it++) {
+      const Conic &A = S.k1, &B = S.k2;
+      double F1 = A.a * x * x + A.b * x * y + A.c * y * y + A.d * x + A.e * y + A.f;
+      double F2 = B.a * x * x + B.b * x * y + B.c * y * y + B.d * x + B.e * y + B.f;
+      double F1x = 2.0 * A.a * x + A.b * y + A.d, F1y = A.b * x + 2.0 * A.c * y + A.e;
+      double F2x = 2.0 * B.a * x + B.b * y + B.d, F2y = B.b * x + 2.0 * B.c * y + B.e;
+      double det = F1x * F2y - F1y * F2x;
+      double dx = (F1 * F2y - F2 * F1y) / det, dy = (F1x * F2 - F2x * F1) / det;
+      if (std::isfinite(dx) && std::isfinite(dy)) { x = x - dx; y = y - dy; }
+    }
     int i = S.n_roots;
     S.x[i] = x; S.y[i] = y;
     double pz = g1.c0 + g1.c1 * x + g1.c2 * y;
     double qx = Mx - x, qy = My - y, qz = g2.c0 + g2.c1 * qx + g2.c2 * qy;
+    S.sz[i] = std::fabs(g1.c0) + std::fabs(g1.c1 * x) + std::fabs(g1.c2 * y);
+    S.szb[i] = std::fabs(g2.c0) + std::fabs(g2.c1 * qx) + std::fabs(g2.c2 * qy);
     S.nu[i] = V4{x, y, pz, std::sqrt(x * x + y * y + pz * pz)};
     S.nub[i] = V4{qx, qy, qz, std::sqrt(qx * qx + qy * qy + qz * qz)};
     double ptn = std::sqrt(x * x + y * y), ptb = std::sqrt(qx * qx + qy * qy);
@@ -292,7 +306,7 @@ void reconstruct_event(const orc_events_t* ev, uint32_t e, int32_t V, uint64_t s
                        orc_best_t* out, orc_aux_t* aux) {
   EventObjects o = load_event(ev, e);
   fill_nan(out); out->event = e; out->status = o.status;
-  if (aux) { aux->kappa = NaN; aux->loglik2 = -INFINITY; aux->n_cand = 0; aux->pairing = aux->higgs_pair = -1; }
+  if (aux) { aux->kappa = NaN; aux->loglik2 = -INFINITY; aux->n_cand = 0; aux->pairing = aux->higgs_pair = -1; aux->pz_terms = aux->pzbar_terms = 0.0; }
   if (!o.applicable) { out->status |= 2u; return; }
   const int nb = o.n_b;
   double best = -INFINITY, second = -INFINITY; bool have = false; int64_t n_cand = 0;
@@ -328,7 +342,7 @@ void reconstruct_event(const orc_events_t* ev, uint32_t e, int32_t V, uint64_t s
             out->m_higgs = mbb; out->loglik = ll;
             out->variation = v; out->jet_b = o.cand[i]; out->jet_bbar = o.cand[j];
             out->jet_h1 = o.cand[k]; out->jet_h2 = o.cand[l]; out->root = r;
-            if (aux) { aux->kappa = S.kappa[r]; aux->pairing = a; aux->higgs_pair = h; }
+            if (aux) { aux->kappa = S.kappa[r]; aux->pairing = a; aux->higgs_pair = h; aux->pz_terms = S.sz[r]; aux->pzbar_terms = S.szb[r]; }
           } else if (ll > second) {
             second = ll;
           }

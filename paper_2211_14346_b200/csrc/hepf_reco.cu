@@ -103,8 +103,8 @@ __device__ __forceinline__ Resultant resultant(const Conic& k1, const Conic& k2)
   return R;
 }
 
-// Real roots of x^4 + g3 x^3 + g2 x^2 + g1 x + g0: Ferrari closed form, then two Newton steps on the quartic.
-// Roots come out as (pair A: x[0], x[1]) then (pair B), unsorted.  Returns 0, 2 or 4.
+// Real roots of x^4 + g3 x^3 + g2 x^2 + g1 x + g0 by Ferrari's closed form (the Newton polish happens in
+// refine_xy, on the pair of conics).  Roots come out as (pair A: x[0], x[1]) then (pair B), unsorted.  Returns 0, 2 or 4.
 __device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, double g0, double (&x)[4]) {
   const double aq = 0.25 * g3, aq2 = aq * aq;
   const double p = g2 - 6.0 * aq2;
@@ -151,17 +151,7 @@ __device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, do
       if (z2 >= 0.0) { const double st = sqrt(z2); t[n++] = st; t[n++] = -st; }
     }
   }
-  for (int k = 0; k < n; k++) {
-    double xx = t[k] - aq;
-#pragma unroll
-    for (int it = 0; it < 2; it++) {
-      const double f = (((xx + g3) * xx + g2) * xx + g1) * xx + g0;
-      const double df = ((4.0 * xx + 3.0 * g3) * xx + 2.0 * g2) * xx + g1;
-      const double step = f / df;
-      if (isfinite(step)) xx -= step;
-    }
-    x[k] = xx;
-  }
+  for (int k = 0; k < n; k++) x[k] = t[k] - aq;
   return n;
 }
 
@@ -177,6 +167,23 @@ __device__ __forceinline__ double root_y(const Resultant& R, const Conic& k1, co
   const double r1 = fabs(k2.a * x * x + k2.b * x * y1 + k2.c * y1 * y1 + k2.d * x + k2.e * y1 + k2.f);
   const double r2 = fabs(k2.a * x * x + k2.b * x * y2 + k2.c * y2 * y2 + k2.d * x + k2.e * y2 + k2.f);
   return r1 <= r2 ? y1 : y2;
+}
+
+// Newton polish of one intersection: start from the Ferrari root x and y = -D1/D2, then two Newton steps on the
+// pair of conics in (x, y).  The quotient alone cancels when D2(x) is small; the 2x2 system is conditioned like
+// the intersection itself (R11a).
+__device__ __forceinline__ void refine_xy(const Resultant& R, const Conic& A, const Conic& B, double& x, double& y) {
+  y = root_y(R, A, B, x);
+#pragma unroll
+  for (int it = 0; it < 2; it++) {
+    const double F1 = (A.a * x + A.b * y + A.d) * x + (A.c * y + A.e) * y + A.f;
+    const double F2 = (B.a * x + B.b * y + B.d) * x + (B.c * y + B.e) * y + B.f;
+    const double F1x = 2.0 * A.a * x + A.b * y + A.d, F1y = A.b * x + 2.0 * A.c * y + A.e;
+    const double F2x = 2.0 * B.a * x + B.b * y + B.d, F2y = B.b * x + 2.0 * B.c * y + B.e;
+    const double idet = 1.0 / (F1x * F2y - F1y * F2x);
+    const double dx = (F1 * F2y - F2 * F1y) * idet, dy = (F1x * F2 - F2x * F1) * idet;
+    if (isfinite(dx) && isfinite(dy)) { x -= dx; y -= dy; }
+  }
 }
 
 struct EventHead {   // what a thread needs to know about its event (uniform over the event's threads)
@@ -335,7 +342,7 @@ reco_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, int V,
               hcount++;
             }
             for (int rr = 0; rr < nr; rr++) {
-              const double xx = x[rr], yy = root_y(R, k1c, k2c, xx);
+              double xx = x[rr], yy; refine_xy(R, k1c, k2c, xx, yy);
               const double qx = S.Mx - xx, qy = S.My - yy;
               const double ptn = sqrt(xx * xx + yy * yy), ptb = sqrt(qx * qx + qy * qy);
               const double ll = ht + (log(ptn * ptb) - (ptn + ptb) * inv_lambda);
@@ -379,13 +386,16 @@ reco_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, int V,
     const Resultant R = resultant(k1c, k2c);
     double x[4];
     const int nr = solve_quartic(R.g3, R.g2, R.g1, R.g0, x);
-    // rank of the winning root among the real roots (ascending); the winner itself is the closest recomputed root
+    // polish every root as the hot loop did; the winner is the recomputed root closest to the remembered one,
+    // its rank is its position among the real roots in ascending order
+    double ys[4];
+    for (int r = 0; r < nr; r++) refine_xy(R, k1c, k2c, x[r], ys[r]);
     int rsel = 0; double dmin = CUDART_INF;
     for (int r = 0; r < nr; r++) { const double d = fabs(x[r] - best.x); if (d < dmin) { dmin = d; rsel = r; } }
     const double xx = (nr > 0) ? x[rsel] : best.x;
+    const double yy = (nr > 0) ? ys[rsel] : CUDART_NAN;
     int rank = 0;
     for (int r = 0; r < nr; r++) rank += (x[r] < xx) || (x[r] == xx && r < rsel);
-    const double yy = root_y(R, k1c, k2c, xx);
     const double pz = c0 + c1 * xx + c2 * yy;
     const double qx = S.Mx - xx, qy = S.My - yy, qz = e0 + e1 * qx + e2 * qy;
     const double en = sqrt(xx * xx + yy * yy + pz * pz), eb = sqrt(qx * qx + qy * qy + qz * qz);
