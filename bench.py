@@ -177,6 +177,7 @@ def main():
     out_cf = torch.zeros(32, dtype=torch.int64, device="cuda")
     ws = torch.empty(int(hepf.load().hepf_select_workspace_bytes(n)) + 256, dtype=torch.uint8, device="cuda")
     out_best = torch.empty((max(n, 1), 128), dtype=torch.uint8, device="cuda")
+    reco_ws = torch.empty(int(hepf.load().hepf_reconstruct_workspace_bytes(n, V)) + 256, dtype=torch.uint8, device="cuda")
     count_host = torch.zeros(1, dtype=torch.int64).pin_memory()
 
     def step(ev_mid=None):
@@ -186,7 +187,7 @@ def main():
         n_sel = int(count_host[0])
         if ev_mid is not None:
             ev_mid[0].record(stream)
-        hepf.reconstruct_tth(dev, out_idx, n_sel, V, seed, out_best=out_best, stream=stream)
+        hepf.reconstruct_tth(dev, out_idx, n_sel, V, seed, out_best=out_best, ws=reco_ws, stream=stream)
         if ev_mid is not None:
             ev_mid[1].record(stream)
         return n_sel

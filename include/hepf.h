@@ -25,7 +25,7 @@ extern "C" {
 #endif
 
 #define HEPF_OK 0
-#define HEPF_ERR_ARG (-1)      /* null / misaligned pointer, negative size, n_cuts > 32, n_variations < 1, odd stride */
+#define HEPF_ERR_ARG (-1)      /* null / misaligned pointer, negative size, n_cuts > 32, n_variations < 1, odd stride, n_variations > 2^21 */
 #define HEPF_ERR_CAPACITY (-2) /* workspace or arena too small                                                    */
 #define HEPF_ERR_CUDA (-3)     /* CUDA runtime / launch failure, or no device                                     */
 
@@ -115,7 +115,8 @@ size_t hepf_select_workspace_bytes(int64_t n_events);
  *   n_idx        host value.
  *   host_params  host pointer or NULL.
  *   out_best     device hepf_best_t[n_idx], 16-byte aligned; out_best[k] belongs to idx[k].
- *   ws           device workspace >= hepf_reconstruct_workspace_bytes(n_idx, n_variations) (may be 0 -> NULL ok).
+ *   ws           device workspace >= hepf_reconstruct_workspace_bytes(n_idx, n_variations), 8-byte aligned (one
+ *                8-byte winner key per listed event, written by the search kernel, read by the finalize kernel).
  */
 int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
                          uint64_t seed, const hepf_tth_params_t* host_params, hepf_best_t* out_best, void* ws,

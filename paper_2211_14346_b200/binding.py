@@ -169,16 +169,19 @@ def select(events: DeviceEvents, chain, *, with_cutflow: bool = True, out_idx=No
 
 
 def reconstruct_tth(events: DeviceEvents, idx, n_idx: int, n_variations: int, seed: int, params: Params | None = None,
-                    *, out_best=None, stream=None):
+                    *, out_best=None, ws=None, stream=None):
     """hepf_reconstruct_tth: returns a uint8 tensor [n_idx, 128] of hepf_best_t records (see BEST_DTYPE)."""
     import torch
     L = load()
     if out_best is None:
         out_best = torch.empty((max(n_idx, 1), 128), dtype=torch.uint8, device=events.cols.device)
+    need = L.hepf_reconstruct_workspace_bytes(max(n_idx, 0), n_variations)
+    if ws is None or ws.numel() < need:
+        ws = torch.empty(max(need, 16), dtype=torch.uint8, device=events.cols.device)
     ev = events.view()
     rc = L.hepf_reconstruct_tth(C.byref(ev), idx.data_ptr(), n_idx, n_variations, seed,
-                                C.byref(params) if params is not None else None, out_best.data_ptr(), None, 0,
-                                _stream_ptr(stream))
+                                C.byref(params) if params is not None else None, out_best.data_ptr(), ws.data_ptr(),
+                                ws.numel(), _stream_ptr(stream))
     _check(rc, "hepf_reconstruct_tth")
     return out_best[:n_idx]
 

@@ -10,6 +10,9 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhepf.so")
 SOURCES = ["hepf_api.cu", "hepf_philox.cu", "hepf_select.cu", "hepf_reco.cu", "hepf_host.cu"]
+# hepf_reco.cu spells every fused multiply-add itself: no contraction, so that the search and the finalize kernel
+# (and any two builds) evaluate the shared device functions to the same bits
+EXTRA_FLAGS = {"hepf_reco.cu": ["-fmad=false"]}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -31,7 +34,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     procs = []
     for s in SOURCES:
         o = os.path.join(HERE, "build", s.replace(".cu", ".o"))
-        cmd = [nvcc, "-c", os.path.join(CSRC, s), "-o", o, "-I", os.path.join(ROOT, "include"), "-I", CSRC] + NVCC_FLAGS
+        cmd = [nvcc, "-c", os.path.join(CSRC, s), "-o", o, "-I", os.path.join(ROOT, "include"), "-I", CSRC] + NVCC_FLAGS + EXTRA_FLAGS.get(s, [])
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(o)
     log = []

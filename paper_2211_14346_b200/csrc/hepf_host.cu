@@ -9,7 +9,7 @@ namespace {
 size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 
 struct ArenaLayout {
-  size_t cols, flags, idx, count, cutflow, sel_ws, best, total;
+  size_t cols, flags, idx, count, cutflow, sel_ws, reco_ws, best, total;
 };
 
 ArenaLayout layout(int64_t n, int64_t stride) {
@@ -21,6 +21,7 @@ ArenaLayout layout(int64_t n, int64_t stride) {
   L.count = off; off += 256;
   L.cutflow = off; off += up256(HEPF_MAX_CUTS * sizeof(int64_t));
   L.sel_ws = off; off += up256(hepf_select_workspace_bytes(n));
+  L.reco_ws = off; off += up256(hepf_reconstruct_workspace_bytes(n, 1));
   L.best = off; off += up256((size_t)(n > 0 ? n : 1) * sizeof(hepf_best_t));
   L.total = off;
   return L;
@@ -87,7 +88,8 @@ extern "C" int hepf_tth_host(const hepf_events_t* hev, const hepf_cut_t* host_cu
   HEPF_CUDA_TRY(cudaMemcpyAsync(host_out_count, dcount, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
   HEPF_CUDA_TRY(cudaStreamSynchronize(stream));
   const int64_t n_sel = *host_out_count;
-  rc = hepf_reconstruct_tth(&dev, didx, n_sel, n_variations, seed, host_params, dbest, nullptr, 0, stream);
+  rc = hepf_reconstruct_tth(&dev, didx, n_sel, n_variations, seed, host_params, dbest, base + L.reco_ws,
+                            up256(hepf_reconstruct_workspace_bytes(n, 1)), stream);
   if (rc != HEPF_OK) return rc;
   if (n_sel > 0) {
     HEPF_CUDA_TRY(cudaMemcpyAsync(host_out_best, dbest, (size_t)n_sel * sizeof(hepf_best_t), cudaMemcpyDeviceToHost, stream));

@@ -6,25 +6,36 @@
 // probable solution wins; PAPER.md:145 — the measured momenta are varied V times within the resolution.  The
 // equations themselves are in DESIGN.md "Method" (the paper defers them to its ref. [27]).
 //
-// B200 mapping (v1): one thread owns one (event, variation).  It draws the ten normals in registers (Philox4x32-10
-// + Box-Muller, bit-identical to the specified operation sequence), smears the objects, builds the n_b leg-2 conics
-// once (kept in a per-thread, bank-conflict-free column of shared memory), then walks the ordered pairings (i, j):
-// leg-1 conic in registers, resultant -> monic quartic -> Ferrari closed form -> two Newton steps per root ->
-// neutrino pT score.  The thread keeps its best candidate; a shared-memory atomicMax/atomicMin pair reduces the
-// threads of one event with the total order (loglik, then lowest (variation, pairing)); the winning thread
-// re-derives the full solution and writes the 128-byte record.  No tensor cores: nothing here is a contraction.
+// B200 mapping (v2).  The work is FP64-pipe bound (no bytes to speak of), so the design goal is: every FP64
+// instruction issued with 32 useful lanes, from a code body small enough to live in the instruction cache.
+//   reco_search_kernel   one WARP per selected event; the V variations are processed in chunks of VC.  Each chunk
+//                        runs a pipeline of short, convergent stages whose work items are spread over the lanes:
+//       A  (variation, Philox block)      -> 2 normals (in-register Philox4x32-10 + Box-Muller) -> 2 scales
+//       M  (variation, x|y)               -> MET' (slot-ordered sum, bit-identical to the definition)
+//       B  (variation, leg, b candidate)  -> leg conic (leg 2 shifted by MET') -> shared-memory table
+//       H  (variation, candidate pair)    -> Higgs mass term
+//       C  (variation, ordered pairing)   -> resultant -> monic quartic -> Ferrari (FP32 seed for the resolvent cubic,
+//                                            FP64 Newton) -> 0/2/4 real roots PUSHED on a per-warp shared-memory stack
+//       D  (one root per lane, popped 32 at a time) -> y, 2 Newton steps on the pair of conics, neutrino-pT score,
+//                                            lane-local best with the total order (loglik, then lowest (v, a, h, root))
+//     Stage D is where SIMT divergence would hurt (62 % / 34 % / 4 % of the wrong pairings have 0 / 2 / 4 roots); the
+//     stack compacts the roots so that D always runs with full warps.  A warp-shuffle argmax ends the event and lane 0
+//     writes an 8-byte winner key to the workspace.  No block-level barrier anywhere: warps drift apart freely, which
+//     keeps the FP64 pipe fed while other warps sit in integer (Philox) or load phases.
+//   reco_finalize_kernel one THREAD per selected event: re-derives the winning (variation, pairing, root) with the same
+//                        device functions (this translation unit is compiled with -fmad=false and spells every fused
+//                        operation, so both kernels produce the same bits) and writes the 128-byte hepf_best_t record.
+// No tensor cores: nothing here is a contraction.
 #include <math_constants.h>
+
+#include <cstdlib>
 
 #include "hepf_common.cuh"
 
 namespace hepf {
 
-constexpr int RECO_THREADS = 128;
-constexpr int NB_MAX = HEPF_MAX_B;
-constexpr int TH_CONIC2 = 0;                      // per-thread shared layout, in doubles
-constexpr int TH_SCALE = TH_CONIC2 + 6 * NB_MAX;  // scales of the b candidates
-constexpr int TH_HT = TH_SCALE + NB_MAX;          // Higgs term of every unordered candidate pair
-constexpr int TH_DOUBLES = TH_HT + 15;
+constexpr int NBM = HEPF_MAX_B;   // candidate slots in the tables
+constexpr int QCAP = 160;         // root stack: <= 31 left over + 32 lanes x 4 new roots
 
 struct RecoCols {
   const double *lep_px, *lep_py, *lep_pz, *lep_e, *jet_px, *jet_py, *jet_pz, *jet_e, *met_x, *met_y;
@@ -35,164 +46,284 @@ struct RecoCols {
 struct V4 { double x, y, z, e; };
 struct Conic { double a, b, c, d, e, f; };
 
-#define SM(k) sm[(k) * RECO_THREADS + threadIdx.x]
-
-__device__ __forceinline__ int tri(int k, int l) { return (k * (11 - k)) / 2 + (l - k - 1); }  // k < l < 6
-
-__device__ __forceinline__ V4 load_v4(const double* px, const double* py, const double* pz, const double* e, int64_t at) {
-  return V4{__ldg(px + at), __ldg(py + at), __ldg(pz + at), __ldg(e + at)};
+// nibble-packed lexicographic lists of the unordered candidate pairs (k < l) for n_b = 4, 5, 6
+__device__ __forceinline__ uint64_t pair_k_list(int nb) {
+  return nb == 4 ? 0x211000ull : (nb == 5 ? 0x3221110000ull : 0x433222111100000ull);
 }
-__device__ __forceinline__ V4 scale_v4(const V4& p, double s) {
-  return V4{__dmul_rn(s, p.x), __dmul_rn(s, p.y), __dmul_rn(s, p.z), __dmul_rn(s, p.e)};
+__device__ __forceinline__ uint64_t pair_l_list(int nb) {
+  return nb == 4 ? 0x332321ull : (nb == 5 ? 0x4434324321ull : 0x554543543254321ull);
+}
+// position of the pair (k, l), k < l < NBT, in the lexicographic list of pairs
+template <int NBT> __device__ __forceinline__ int pair_index(int k, int l) { return (k * (2 * NBT - 1 - k)) / 2 + (l - k - 1); }
+
+// ---- branch-free FP64 reciprocal / square root / logarithm for the tolerance-compared part of the path ------------
+// MUFU seed (2^-20, measured on B200) + one cubic (rcp) or two quadratic (sqrt) correction steps: <= 1 ulp (rcp) and
+// correctly rounded in every sampled case (sqrt), with 4 resp. 7 FP64-pipe instructions and no slow-path branch.  The
+// smearing (normals, scales, MET') does NOT use these: it keeps the IEEE operations the definition prescribes.
+__device__ __forceinline__ double rcp_fast(double b) {
+  double r; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+  const double e = fma(-b, r, 1.0);
+  return fma(r, fma(e, e, e), r);
+}
+__device__ __forceinline__ double sqrt_fast(double a) {
+  double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+  double h = 0.5 * y, s = a * y;
+  const double e = fma(-s, h, 0.5);
+  s = fma(s, e, s); h = fma(h, e, h);
+  s = fma(fma(-s, s, a), h, s);
+  return a == 0.0 ? 0.0 : s;
+}
+// ln(a), a > 0 normal: a = m 2^e with m in (sqrt(1/2), sqrt(2)], ln m = 2 atanh(s), s = (m-1)/(m+1); error < 3e-16 relative
+__device__ __forceinline__ double ln_fast(double a) {
+  int hi = __double2hiint(a);
+  int e = ((hi >> 20) & 0x7ff) - 1023;
+  double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(a));
+  if (m > 0x1.6a09e667f3bcdp+0) { m *= 0.5; e += 1; }
+  const double f = m - 1.0, s = f * rcp_fast(2.0 + f), z = s * s;
+  double p = 2.0 / 19.0;
+  p = fma(p, z, 2.0 / 17.0); p = fma(p, z, 2.0 / 15.0); p = fma(p, z, 2.0 / 13.0); p = fma(p, z, 2.0 / 11.0);
+  p = fma(p, z, 2.0 / 9.0); p = fma(p, z, 2.0 / 7.0); p = fma(p, z, 2.0 / 5.0); p = fma(p, z, 2.0 / 3.0);
+  const double lm = fma(s, p * z, 2.0 * s), ed = (double)e;
+  const double r = fma(ed, 0x1.62e42fee00000p-1, fma(ed, 0x1.a39ef35793c76p-33, lm));
+  return a > 0.0 ? r : (a == 0.0 ? -CUDART_INF : CUDART_NAN);
+}
+
+__device__ __forceinline__ V4 scale_v4(const double* p, double s) {
+  return V4{__dmul_rn(s, p[0]), __dmul_rn(s, p[1]), __dmul_rn(s, p[2]), __dmul_rn(s, p[3])};
 }
 __device__ __forceinline__ double mass_of(double e, double x, double y, double z) {
-  const double m2 = e * e - (x * x + y * y + z * z);
-  return sqrt(m2 > 0.0 ? m2 : 0.0);
+  const double m2 = fma(e, e, -fma(x, x, fma(y, y, z * z)));
+  return sqrt_fast(m2 > 0.0 ? m2 : 0.0);
 }
 
 // Leg conic of (lepton l, b-jet b): neutrino p_z = c0 + c1 p_x + c2 p_y and the conic in (p_x, p_y).
 __device__ __forceinline__ bool leg_conic(const V4& l, const V4& b, double mt2, double mw2, Conic& q, double& c0,
                                           double& c1, double& c2) {
-  const double ml2 = l.e * l.e - (l.x * l.x + l.y * l.y + l.z * l.z);
-  const double mb2 = b.e * b.e - (b.x * b.x + b.y * b.y + b.z * b.z);
-  const double bl = b.e * l.e - (b.x * l.x + b.y * l.y + b.z * l.z);
+  const double ml2 = fma(l.e, l.e, -fma(l.x, l.x, fma(l.y, l.y, l.z * l.z)));
+  const double mb2 = fma(b.e, b.e, -fma(b.x, b.x, fma(b.y, b.y, b.z * b.z)));
+  const double bl = fma(b.e, l.e, -fma(b.x, l.x, fma(b.y, l.y, b.z * l.z)));
   const double A = 0.5 * (mw2 - ml2);
-  const double B = 0.5 * (mt2 - mw2 - mb2) - bl;
-  const double nx = b.e * l.x - l.e * b.x, ny = b.e * l.y - l.e * b.y, nz = b.e * l.z - l.e * b.z;
-  const double k = l.e * B - b.e * A;
+  const double B = fma(0.5, (mt2 - mw2) - mb2, -bl);
+  const double nx = fma(b.e, l.x, -(l.e * b.x)), ny = fma(b.e, l.y, -(l.e * b.y)), nz = fma(b.e, l.z, -(l.e * b.z));
+  const double k = fma(l.e, B, -(b.e * A));
   const bool ok = fabs(nz) > 1e-12 * b.e * l.e;
-  const double inz = 1.0 / nz, ile = 1.0 / l.e;
+  const double inz = rcp_fast(nz), ile = rcp_fast(l.e);
   c0 = k * inz; c1 = -nx * inz; c2 = -ny * inz;
-  const double d0 = (A + l.z * c0) * ile, d1 = (l.x + l.z * c1) * ile, d2 = (l.y + l.z * c2) * ile;
-  q.a = d1 * d1 - 1.0 - c1 * c1;
-  q.b = 2.0 * (d1 * d2 - c1 * c2);
-  q.c = d2 * d2 - 1.0 - c2 * c2;
-  q.d = 2.0 * (d0 * d1 - c0 * c1);
-  q.e = 2.0 * (d0 * d2 - c0 * c2);
-  q.f = d0 * d0 - c0 * c0;
+  const double d0 = fma(l.z, c0, A) * ile, d1 = fma(l.z, c1, l.x) * ile, d2 = fma(l.z, c2, l.y) * ile;
+  q.a = fma(d1, d1, -fma(c1, c1, 1.0));
+  q.b = 2.0 * fma(d1, d2, -(c1 * c2));
+  q.c = fma(d2, d2, -fma(c2, c2, 1.0));
+  q.d = 2.0 * fma(d0, d1, -(c0 * c1));
+  q.e = 2.0 * fma(d0, d2, -(c0 * c2));
+  q.f = fma(d0, d0, -(c0 * c0));
   return ok;
 }
 
+// the conic of leg 2 is in q = MET' - p; rewrite it in p
 __device__ __forceinline__ Conic shift_conic(const Conic& q, double Mx, double My) {
   Conic s;
   s.a = q.a; s.b = q.b; s.c = q.c;
-  s.d = -2.0 * q.a * Mx - q.b * My - q.d;
-  s.e = -2.0 * q.c * My - q.b * Mx - q.e;
-  s.f = q.a * Mx * Mx + q.b * Mx * My + q.c * My * My + q.d * Mx + q.e * My + q.f;
+  const double tx = fma(q.a, Mx, fma(q.b, My, q.d)), ty = fma(q.c, My, q.e);
+  s.d = -fma(q.a, Mx, tx);                 // -(2 a Mx + b My + d)
+  s.e = -fma(q.b, Mx, fma(q.c, My, ty));   // -(2 c My + b Mx + e)
+  s.f = fma(tx, Mx, fma(ty, My, q.f));
   return s;
 }
 
-struct Resultant { double p0, p1, p2, q0, q1, g0, g1, g2, g3; };
-
-// resultant of the two conics in x (y eliminated) as a MONIC quartic g, plus D1 = p0+p1x+p2x^2, D2 = q0+q1x
-__device__ __forceinline__ Resultant resultant(const Conic& k1, const Conic& k2) {
-  Resultant R;
-  R.p0 = k1.c * k2.f - k2.c * k1.f; R.p1 = k1.c * k2.d - k2.c * k1.d; R.p2 = k1.c * k2.a - k2.c * k1.a;
-  R.q0 = k1.c * k2.e - k2.c * k1.e; R.q1 = k1.c * k2.b - k2.c * k1.b;
-  const double r0 = k1.e * k2.f - k2.e * k1.f;
-  const double r1 = k1.e * k2.d + k1.b * k2.f - k2.e * k1.d - k2.b * k1.f;
-  const double r2 = k1.e * k2.a + k1.b * k2.d - k2.e * k1.a - k2.b * k1.d;
-  const double r3 = k1.b * k2.a - k2.b * k1.a;
-  const double h0 = R.p0 * R.p0 - R.q0 * r0;
-  const double h1 = 2.0 * R.p0 * R.p1 - (R.q0 * r1 + R.q1 * r0);
-  const double h2 = 2.0 * R.p0 * R.p2 + R.p1 * R.p1 - (R.q0 * r2 + R.q1 * r1);
-  const double h3 = 2.0 * R.p1 * R.p2 - (R.q0 * r3 + R.q1 * r2);
-  const double h4 = R.p2 * R.p2 - R.q1 * r3;
-  const double ih4 = 1.0 / h4;   // h4 == 0 -> inf/NaN coefficients -> every discriminant test below is false
-  R.g0 = h0 * ih4; R.g1 = h1 * ih4; R.g2 = h2 * ih4; R.g3 = h3 * ih4;
-  return R;
+struct Lines { double p0, p1, p2, q0, q1; };   // D1(x) = p0 + p1 x + p2 x^2, D2(x) = q0 + q1 x
+__device__ __forceinline__ Lines lines_of(const Conic& k1, const Conic& k2) {
+  Lines L;
+  L.p0 = fma(k1.c, k2.f, -(k2.c * k1.f)); L.p1 = fma(k1.c, k2.d, -(k2.c * k1.d)); L.p2 = fma(k1.c, k2.a, -(k2.c * k1.a));
+  L.q0 = fma(k1.c, k2.e, -(k2.c * k1.e)); L.q1 = fma(k1.c, k2.b, -(k2.c * k1.b));
+  return L;
 }
 
-// Real roots of x^4 + g3 x^3 + g2 x^2 + g1 x + g0 by Ferrari's closed form (the Newton polish happens in
-// refine_xy, on the pair of conics).  Roots come out as (pair A: x[0], x[1]) then (pair B), unsorted.  Returns 0, 2 or 4.
-__device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, double g0, double (&x)[4]) {
-  const double aq = 0.25 * g3, aq2 = aq * aq;
-  const double p = g2 - 6.0 * aq2;
-  const double q = g1 - 2.0 * aq * g2 + 8.0 * aq2 * aq;
-  const double r = g0 - aq * g1 + aq2 * g2 - 3.0 * aq2 * aq2;
-  // resolvent cubic m^3 + p m^2 + (p^2/4 - r) m - q^2/8 = 0, largest real root (>= 0)
-  const double c1 = 0.25 * p * p - r, c0 = -0.125 * q * q;
-  const double p3 = p * (1.0 / 3.0);
-  const double P = c1 - p * p3;
-  const double Q = 2.0 * p3 * p3 * p3 - p3 * c1 + c0;
-  const double u = -0.5 * Q, P3 = P * (1.0 / 3.0);
-  const double D = u * u + P3 * P3 * P3;
-  double w;
-  if (D > 0.0) {
-    const double sD = sqrt(D);
-    const double A = (u >= 0.0) ? cbrt(u + sD) : -cbrt(sD - u);
-    w = (A != 0.0) ? A - P3 / A : 0.0;
+// resultant of the two conics in x (y eliminated) as a MONIC quartic x^4 + g3 x^3 + g2 x^2 + g1 x + g0
+__device__ __forceinline__ void resultant(const Conic& k1, const Conic& k2, double& g3, double& g2, double& g1, double& g0) {
+  const Lines L = lines_of(k1, k2);
+  const double r0 = fma(k1.e, k2.f, -(k2.e * k1.f));
+  const double r1 = fma(k1.e, k2.d, fma(k1.b, k2.f, -fma(k2.e, k1.d, k2.b * k1.f)));
+  const double r2 = fma(k1.e, k2.a, fma(k1.b, k2.d, -fma(k2.e, k1.a, k2.b * k1.d)));
+  const double r3 = fma(k1.b, k2.a, -(k2.b * k1.a));
+  const double tp0 = 2.0 * L.p0, tp1 = 2.0 * L.p1;
+  const double h0 = fma(L.p0, L.p0, -(L.q0 * r0));
+  const double h1 = fma(tp0, L.p1, -fma(L.q0, r1, L.q1 * r0));
+  const double h2 = fma(tp0, L.p2, fma(L.p1, L.p1, -fma(L.q0, r2, L.q1 * r1)));
+  const double h3 = fma(tp1, L.p2, -fma(L.q0, r3, L.q1 * r2));
+  const double h4 = fma(L.p2, L.p2, -(L.q1 * r3));
+  const double ih4 = rcp_fast(h4);   // h4 == 0 -> inf/NaN coefficients -> every discriminant test below is false
+  g0 = h0 * ih4; g1 = h1 * ih4; g2 = h2 * ih4; g3 = h3 * ih4;
+}
+
+__device__ __forceinline__ int exp_of(double v) { return ((__double2hiint(v) >> 20) & 0x7ff) - 1023; }
+__device__ __forceinline__ double pow2(int e) { return __hiloint2double((1023 + e) << 20, 0); }   // -1022 <= e <= 1023
+
+// cos(acos(c) / 3) for c in [-1, 1], FP32, ~1e-6: acos(|c|) = sqrt(1 - |c|) * poly(|c|) (Abramowitz & Stegun 4.4.46,
+// |error| <= 2e-8), reflected for c < 0; then the cosine series on [0, pi/3].  No libm call: only a seed is needed.
+__device__ __forceinline__ float cos_third_acos(float c) {
+  const float a = fabsf(c);
+  float p = -0.0012624911f;
+  p = fmaf(p, a, 0.0066700901f); p = fmaf(p, a, -0.0170881256f); p = fmaf(p, a, 0.0308918810f);
+  p = fmaf(p, a, -0.0501743046f); p = fmaf(p, a, 0.0889789874f); p = fmaf(p, a, -0.2145988016f);
+  p = fmaf(p, a, 1.5707963050f);
+  float phi = sqrtf(1.0f - a) * p;
+  phi = (c < 0.0f) ? 3.14159265f - phi : phi;
+  const float t = phi * (1.0f / 3.0f), z = t * t;
+  float q = -1.0f / 3628800.0f;
+  q = fmaf(q, z, 1.0f / 40320.0f); q = fmaf(q, z, -1.0f / 720.0f); q = fmaf(q, z, 1.0f / 24.0f); q = fmaf(q, z, -0.5f);
+  return fmaf(q, z, 1.0f);
+}
+
+// Seed for the largest real root of the resolvent cubic m^3 + p m^2 + (p^2/4 - r) m - q^2/8 = 0: the closed form
+// (Cardano / trigonometric) evaluated in FP32 on the FP32 pipe, after an exact power-of-two rescaling t = 2^E tau that
+// brings the depressed quartic's coefficients to O(1).  Only a starting point: FP64 Newton steps follow.
+__device__ __forceinline__ double resolvent_seed(double p, double q, double r) {
+  int E = max(max((exp_of(p) + 1) >> 1, (exp_of(q) + 2) / 3), (exp_of(r) + 3) >> 2);
+  E = min(250, max(-250, E));
+  const float pf = (float)(p * pow2(-2 * E)), qf = (float)(q * pow2(-3 * E)), rf = (float)(r * pow2(-4 * E));
+  const float c1 = fmaf(0.25f * pf, pf, -rf), c0 = -0.125f * qf * qf;
+  const float p3 = pf * (1.0f / 3.0f);
+  const float P3 = (c1 - pf * p3) * (1.0f / 3.0f);
+  const float u = -0.5f * fmaf(2.0f * p3 * p3, p3, fmaf(-p3, c1, c0));
+  const float D = fmaf(u, u, P3 * P3 * P3);
+  float w;
+  if (D > 0.0f) {
+    const float A = cbrtf(u + copysignf(sqrtf(D), u));
+    w = (A != 0.0f) ? A - P3 / A : 0.0f;
   } else {
-    const double rho = sqrt(-P3);
-    double ct = u / (rho * rho * rho);
-    ct = fmin(1.0, fmax(-1.0, ct));
-    w = (rho > 0.0) ? 2.0 * rho * cos(acos(ct) * (1.0 / 3.0)) : 0.0;
+    const float rho = sqrtf(-P3);
+    const float ct = fminf(1.0f, fmaxf(-1.0f, u / (rho * rho * rho)));
+    w = (rho > 0.0f) ? 2.0f * rho * cos_third_acos(ct) : 0.0f;
   }
-  double m = w - p3;
-#pragma unroll
-  for (int it = 0; it < 2; it++) {   // Newton on the resolvent: removes the closed form's cancellation error
-    const double f = ((m + p) * m + c1) * m + c0, df = (3.0 * m + 2.0 * p) * m + c1;
+  return (double)(w - p3) * pow2(2 * E);
+}
+
+// Largest real root of m^3 + p m^2 + c1 m + c0 (c0 <= 0, so it is >= 0) by Newton from an upper bound of all roots: the
+// iterates decrease monotonically onto it.  Slow path of solve_quartic; NaN coefficients fall through and return NaN.
+__device__ __noinline__ double resolvent_root_from_above(double p, double tp, double c1, double c0) {
+  const int E = max(max(exp_of(p) + 1, (exp_of(c1) + 2) >> 1), (exp_of(c0) + 3) / 3) + 1;   // 2 max(|p|, |c1|^1/2, |c0|^1/3) <= 2^E
+  double m = pow2(min(1000, max(-1000, E)));
+#pragma unroll 1
+  for (int it = 0; it < 200; it++) {
+    const double f = fma(fma(m + p, m, c1), m, c0), df = fma(fma(3.0, m, tp), m, c1);
     const double step = f / df;
-    if (isfinite(step)) m -= step;
+    if (!(step > 0.0)) break;              // at the root (f <= 0 by rounding), or NaN
+    m -= step;
+    if (step <= 1e-15 * m) break;
   }
-  int n = 0;
-  double t[4];
+  return m;
+}
+
+struct Biquad { double x[4]; int mask; };
+__device__ __noinline__ Biquad biquadratic_roots(double p, double r, double aq) {
+  Biquad b; b.mask = 0; b.x[0] = b.x[1] = b.x[2] = b.x[3] = 0.0;
+  const double dz = fma(p, p, -4.0 * r);
+  if (dz >= 0.0) {
+    const double sq = sqrt(dz), z1 = 0.5 * (sq - p), z2 = -0.5 * (p + sq);
+    if (z1 >= 0.0) { const double st = sqrt(z1); b.x[0] = st - aq; b.x[1] = -st - aq; b.mask |= 1; }
+    if (z2 >= 0.0) { const double st = sqrt(z2); b.x[2] = st - aq; b.x[3] = -st - aq; b.mask |= 2; }
+  }
+  return b;
+}
+
+// Real roots of x^4 + g3 x^3 + g2 x^2 + g1 x + g0 by Ferrari's closed form; the polish happens later, on the pair of
+// conics.  Roots come out as pair A (xa[0], xa[1]) and pair B (xb[0], xb[1]).  Returns bit 0 = pair A real, bit 1 = B.
+__device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, double g0, double (&xa)[2], double (&xb)[2]) {
+  const double aq = 0.25 * g3, aq2 = aq * aq;
+  const double p = fma(-6.0, aq2, g2);
+  const double q = fma(aq, fma(8.0, aq2, -2.0 * g2), g1);
+  const double r = fma(aq2, fma(-3.0, aq2, g2), fma(-aq, g1, g0));
+  const double c1 = fma(0.25 * p, p, -r), c0 = -0.125 * q * q, tp = 2.0 * p;
+  double m = resolvent_seed(p, q, r), step = 0.0;
+#pragma unroll
+  for (int it = 0; it < 3; it++) {   // FP64 Newton on the resolvent cubic
+    const double f = fma(fma(m + p, m, c1), m, c0), df = fma(fma(3.0, m, tp), m, c1);
+    step = f * rcp_fast(df);
+    m -= step;
+  }
+  // The seed is only FP32: accept the iterate if the last step was a converged one onto a positive root (any positive
+  // root of the resolvent gives a real factorisation); otherwise take the slow, monotone route (rare).
+  if (!(fabs(step) <= 1e-8 * m)) m = resolvent_root_from_above(p, tp, c1, c0);
+  int mask = 0;
   if (m > 0.0) {
-    const double s = sqrt(2.0 * m), qs = q / (2.0 * s);
+    const double s = sqrt_fast(2.0 * m), qs = q * rcp_fast(s);          // 2 qs' with qs' = q / (2 s)
     const double base = -2.0 * (m + p);
-    const double dA = base - 4.0 * qs, dB = base + 4.0 * qs;
-    if (dA >= 0.0) { const double sq = sqrt(dA); t[n++] = 0.5 * (s + sq); t[n++] = 0.5 * (s - sq); }
-    if (dB >= 0.0) { const double sq = sqrt(dB); t[n++] = 0.5 * (-s + sq); t[n++] = 0.5 * (-s - sq); }
-  } else if (m == m) {               // q == 0 up to rounding: biquadratic t^4 + p t^2 + r
-    const double dz = p * p - 4.0 * r;
-    if (dz >= 0.0) {
-      const double sq = sqrt(dz), z1 = 0.5 * (-p + sq), z2 = 0.5 * (-p - sq);
-      if (z1 >= 0.0) { const double st = sqrt(z1); t[n++] = st; t[n++] = -st; }
-      if (z2 >= 0.0) { const double st = sqrt(z2); t[n++] = st; t[n++] = -st; }
-    }
+    const double dA = fma(-2.0, qs, base), dB = fma(2.0, qs, base);
+    if (dA >= 0.0) { const double sq = sqrt_fast(dA); xa[0] = fma(0.5, s + sq, -aq); xa[1] = fma(0.5, s - sq, -aq); mask |= 1; }
+    if (dB >= 0.0) { const double sq = sqrt_fast(dB); xb[0] = fma(0.5, sq - s, -aq); xb[1] = fma(-0.5, s + sq, -aq); mask |= 2; }
+  } else if (m == m) {               // q == 0 up to rounding: biquadratic t^4 + p t^2 + r (rare, out of line)
+    const Biquad b = biquadratic_roots(p, r, aq);
+    xa[0] = b.x[0]; xa[1] = b.x[1]; xb[0] = b.x[2]; xb[1] = b.x[3]; mask = b.mask;
   }
-  for (int k = 0; k < n; k++) x[k] = t[k] - aq;
-  return n;
+  return mask;
+}
+
+__device__ __forceinline__ double conic_at(const Conic& k, double x, double y) {
+  return fma(fma(k.a, x, fma(k.b, y, k.d)), x, fma(fma(k.c, y, k.e), y, k.f));
 }
 
 // y of a root x: y = -D1(x)/D2(x); when the conics share the y direction at x, solve conic 1 and keep the
 // y closer to conic 2 (step 3).
-__device__ __forceinline__ double root_y(const Resultant& R, const Conic& k1, const Conic& k2, double x) {
-  const double D1 = R.p0 + x * (R.p1 + x * R.p2), D2 = R.q0 + R.q1 * x;
-  if (fabs(D2) > 1e-12 * (fabs(R.q0) + fabs(R.q1 * x))) return -D1 / D2;
-  const double qa = k1.c, qb = k1.b * x + k1.e, qc = (k1.a * x + k1.d) * x + k1.f;
-  const double dd = qb * qb - 4.0 * qa * qc;
+__device__ __noinline__ double root_y_fallback(const Conic k1, const Conic k2, double x) {
+  const double qa = k1.c, qb = fma(k1.b, x, k1.e), qc = fma(fma(k1.a, x, k1.d), x, k1.f);
+  const double dd = fma(qb, qb, -4.0 * qa * qc);
   if (!(dd >= 0.0) || qa == 0.0) return CUDART_NAN;
   const double sq = sqrt(dd), y1 = (-qb - sq) / (2.0 * qa), y2 = (-qb + sq) / (2.0 * qa);
-  const double r1 = fabs(k2.a * x * x + k2.b * x * y1 + k2.c * y1 * y1 + k2.d * x + k2.e * y1 + k2.f);
-  const double r2 = fabs(k2.a * x * x + k2.b * x * y2 + k2.c * y2 * y2 + k2.d * x + k2.e * y2 + k2.f);
-  return r1 <= r2 ? y1 : y2;
+  return fabs(conic_at(k2, x, y1)) <= fabs(conic_at(k2, x, y2)) ? y1 : y2;
 }
 
-// Newton polish of one intersection: start from the Ferrari root x and y = -D1/D2, then two Newton steps on the
-// pair of conics in (x, y).  The quotient alone cancels when D2(x) is small; the 2x2 system is conditioned like
-// the intersection itself (R11a).
-__device__ __forceinline__ void refine_xy(const Resultant& R, const Conic& A, const Conic& B, double& x, double& y) {
-  y = root_y(R, A, B, x);
-#pragma unroll
-  for (int it = 0; it < 2; it++) {
-    const double F1 = (A.a * x + A.b * y + A.d) * x + (A.c * y + A.e) * y + A.f;
-    const double F2 = (B.a * x + B.b * y + B.d) * x + (B.c * y + B.e) * y + B.f;
-    const double F1x = 2.0 * A.a * x + A.b * y + A.d, F1y = A.b * x + 2.0 * A.c * y + A.e;
-    const double F2x = 2.0 * B.a * x + B.b * y + B.d, F2y = B.b * x + 2.0 * B.c * y + B.e;
-    const double idet = 1.0 / (F1x * F2y - F1y * F2x);
-    const double dx = (F1 * F2y - F2 * F1y) * idet, dy = (F1x * F2 - F2x * F1) * idet;
-    if (isfinite(dx) && isfinite(dy)) { x -= dx; y -= dy; }
+// one Newton step on the pair of conics in (x, y); mv = |dx| + |dy| (left unchanged, and the point kept, if the
+// Jacobian is singular)
+__device__ __forceinline__ void newton_xy(const Conic& A, const Conic& B, double& x, double& y, double& mv) {
+  const double t1 = fma(A.a, x, fma(A.b, y, A.d)), t2 = fma(A.c, y, A.e);
+  const double F1 = fma(t1, x, fma(t2, y, A.f)), F1x = fma(A.a, x, t1), F1y = fma(A.b, x, fma(A.c, y, t2));
+  const double u1 = fma(B.a, x, fma(B.b, y, B.d)), u2 = fma(B.c, y, B.e);
+  const double F2 = fma(u1, x, fma(u2, y, B.f)), F2x = fma(B.a, x, u1), F2y = fma(B.b, x, fma(B.c, y, u2));
+  const double idet = rcp_fast(fma(F1x, F2y, -(F1y * F2x)));
+  const double dx = fma(F1, F2y, -(F2 * F1y)) * idet, dy = fma(F1x, F2, -(F2x * F1)) * idet;
+  const double m = fabs(dx) + fabs(dy);
+  const bool fin = m <= CUDART_MAX_NORMAL_F;
+  x = fin ? x - dx : x; y = fin ? y - dy : y; mv = fin ? m : 0.0;
+}
+__device__ __noinline__ double2 refine_more(const Conic A, const Conic B, double x, double y) {
+#pragma unroll 1
+  for (int it = 0; it < 6; it++) {
+    double mv = 0.0;
+    newton_xy(A, B, x, y, mv);
+    if (mv <= 1e-10 * (fabs(x) + fabs(y))) break;
   }
+  return make_double2(x, y);
 }
 
-struct EventHead {   // what a thread needs to know about its event (uniform over the event's threads)
+// One intersection: start from the Ferrari root x and y = -D1/D2, then two Newton steps on the pair of conics in
+// (x, y).  The quotient alone cancels when D2(x) is small; the 2x2 system is conditioned like the intersection
+// itself (R11a).
+__device__ __forceinline__ void refine_xy(const Conic& A, const Conic& B, double& x, double& y) {
+  const Lines L = lines_of(A, B);
+  const double D1 = fma(fma(L.p2, x, L.p1), x, L.p0), q1x = L.q1 * x, D2 = L.q0 + q1x;
+  if (fabs(D2) > 1e-12 * (fabs(L.q0) + fabs(q1x))) y = -D1 * rcp_fast(D2);
+  else y = root_y_fallback(A, B, x);
+  double mv = 0.0;
+#pragma unroll
+  for (int it = 0; it < 2; it++) newton_xy(A, B, x, y, mv);
+  // a second step that still moved the point by more than 1e-10 (relative) means near-tangent conics (linear
+  // convergence): keep polishing out of line, up to six more steps
+  if (mv > 1e-10 * (fabs(x) + fabs(y))) { const double2 r = refine_more(A, B, x, y); x = r.x; y = r.y; }
+}
+
+// log-likelihood of one refined root (Higgs term ht already chosen)
+__device__ __forceinline__ double loglik_of(double x, double y, double Mx, double My, double ht, double inv_lambda) {
+  const double qx = Mx - x, qy = My - y;
+  const double ptn = sqrt_fast(fma(x, x, y * y)), ptb = sqrt_fast(fma(qx, qx, qy * qy));
+  return ht + fma(-(ptn + ptb), inv_lambda, ln_fast(ptn * ptb));
+}
+
+struct EventHead {   // what a warp / thread needs to know about its event
   int64_t e;         // index inside the view
   uint64_t gidx;     // global index (keys the smearing stream)
   uint32_t status;
-  int n_jet, n_b, lp_slot;
+  int n_jet, n_b, lp_slot, nblk;
   uint32_t cand;     // candidate jet slots, one nibble each
-  uint32_t pos;      // for each jet slot: its candidate position (nibble), 15 = not a candidate
   bool applicable;
 };
 
@@ -203,227 +334,387 @@ __device__ __forceinline__ EventHead load_head(const RecoCols& ev, int64_t e) {
   const int n_lep = f & 15u;
   h.n_jet = min(8u, (f >> 8) & 15u);
   const bool q0 = (f >> 4) & 1u, q1 = (f >> 5) & 1u;
-  h.cand = 0; h.pos = 0xffffffffu; h.n_b = 0; h.status = 0;
-  int n_tag = 0;
-#pragma unroll
-  for (int s = 0; s < HEPF_N_JET; s++) {
-    if (s < h.n_jet && ((f >> (16 + s)) & 1u)) {
-      if (h.n_b < NB_MAX) {
-        h.cand |= (uint32_t)s << (4 * h.n_b);
-        h.pos = (h.pos & ~(15u << (4 * s))) | ((uint32_t)h.n_b << (4 * s));
-        h.n_b++;
-      }
-      n_tag++;
-    }
+  h.cand = 0; h.n_b = 0; h.status = 0;
+  uint32_t tags = (f >> 16) & ((1u << h.n_jet) - 1u);
+  const int n_tag = __popc(tags);
+  for (int c = 0; c < NBM && tags; c++) {
+    const int s = __ffs(tags) - 1; tags &= tags - 1;
+    h.cand |= (uint32_t)s << (4 * c); h.n_b++;
   }
-  if (n_tag > NB_MAX) h.status |= 4u;
+  if (n_tag > NBM) h.status |= 4u;
   h.applicable = (n_lep == 2) && (q0 != q1) && (h.n_b >= 4);
   if (!h.applicable) h.status |= 2u;
   h.lp_slot = q0 ? 0 : 1;
+  h.nblk = (2 + h.n_jet + 1) >> 1;   // Philox blocks whose normals are used (objects 0 .. 1 + n_jet)
   return h;
 }
 
-struct Smeared { V4 lp, lm; double Mx, My; };
+// nominal object t (0,1 leptons; 2+j jet slot j) and its kappa*sigma (step 2)
+__device__ __forceinline__ void load_object(const RecoCols& ev, int64_t e, int t, const hepf_tth_params_t& P, double* obj4,
+                                            double& ks) {
+  const int64_t at = (t < 2 ? t : t - 2) * ev.stride + e;
+  const double *px = t < 2 ? ev.lep_px : ev.jet_px, *py = t < 2 ? ev.lep_py : ev.jet_py;
+  const double *pz = t < 2 ? ev.lep_pz : ev.jet_pz, *pe = t < 2 ? ev.lep_e : ev.jet_e;
+  obj4[0] = __ldg(px + at); obj4[1] = __ldg(py + at); obj4[2] = __ldg(pz + at); obj4[3] = __ldg(pe + at);
+  const double sigma = t < 2 ? P.lep_sigma : __dadd_rn(__ddiv_rn(P.jet_stoch, __dsqrt_rn(obj4[3])), P.jet_const);
+  ks = __dmul_rn(P.sigma_scale, sigma);
+}
+__device__ __forceinline__ double scale_of(double ks, double z, double s_min) {
+  const double sc = __fma_rn(ks, z, 1.0);
+  return sc > s_min ? sc : s_min;
+}
 
-// Normals, scales, MET' of one (event, variation); candidate scales go to the thread's shared column.
-__device__ __forceinline__ Smeared smear_variation(const RecoCols& ev, const EventHead& h, int v, uint32_t k0, uint32_t k1,
-                                                  const hepf_tth_params_t& P, double* sm) {
-  double z[10];
+// winner key: (variation, pairing i*6+j, Higgs pair, Ferrari slot) in enumeration order; smaller = earlier
+__device__ __forceinline__ uint32_t make_key(int v, int i, int j, int h, int k) {
+  return ((uint32_t)v << 11) | ((uint32_t)(i * 6 + j) << 5) | ((uint32_t)h << 2) | (uint32_t)k;
+}
+
+// best Higgs pair for the pairing (i, j): candidates not in {i, j}, lexicographic order, first maximum of the term
+template <int NBT, int VC>
+__device__ __forceinline__ void best_higgs(const double* ht15, int nb, int i, int j, double& ht, int& h, int& kk, int& ll) {
+  uint32_t rem = ((1u << nb) - 1u) & ~(1u << i) & ~(1u << j);
+  int r[4], nr = 0;
 #pragma unroll
-  for (int blk = 0; blk < 5; blk++) {
-    uint32_t x[4];
-    philox4x32_10((uint32_t)h.gidx, (uint32_t)(h.gidx >> 32), (uint32_t)v, 0x54544800u + blk, k0, k1, x);
-    block_normals(x, z[2 * blk], z[2 * blk + 1]);
+  for (int c = 0; c < 4; c++) { r[c] = __ffs(rem) - 1; nr += rem != 0; rem &= rem - 1; }
+  ht = -CUDART_INF; h = 0; kk = r[0]; ll = r[1];
+  int hc = 0;
+#pragma unroll
+  for (int a = 0; a < 3; a++)
+#pragma unroll
+    for (int b = a + 1; b < 4; b++) {
+      if (b < nr) {
+        const double t = ht15[pair_index<NBT>(r[a], r[b]) * VC];
+        if (t > ht) { ht = t; h = hc; kk = r[a]; ll = r[b]; }
+        hc++;
+      }
+    }
+}
+
+template <int VC, int NBT>
+struct __align__(16) WarpMem {
+  static constexpr int NP = NBT * (NBT - 1) / 2;
+  double con[6][2 * NBT * VC];   // [coefficient][(leg, candidate, variation)]: lanes of a pass differ in the variation
+  double ht[VC * NP];            // Higgs term of candidate pair (k, l), k < l
+  double sc[VC * 10];            // scales of the ten objects
+  double M[VC * 2];              // MET'
+  double obj[10 * 4];            // nominal (px, py, pz, E)
+  double ks[10];                 // kappa * sigma
+  double met[2];
+  double qx[QCAP];               // root stack
+  uint32_t qtag[QCAP];
+};
+
+template <int VC, int NBT>
+__device__ __forceinline__ void score_entry(const WarpMem<VC, NBT>& W, double x, uint32_t tag, int v0, double inv_lambda,
+                                            double& best_ll, uint32_t& best_key) {
+  const int vv = tag & 31, i = (tag >> 5) & 7, j = (tag >> 8) & 7, h = (tag >> 11) & 7, t = (tag >> 14) & 15, k = (tag >> 18) & 3;
+  const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
+  const Conic A{W.con[0][a1], W.con[1][a1], W.con[2][a1], W.con[3][a1], W.con[4][a1], W.con[5][a1]};
+  const Conic B{W.con[0][a2], W.con[1][a2], W.con[2][a2], W.con[3][a2], W.con[4][a2], W.con[5][a2]};
+  double y;
+  refine_xy(A, B, x, y);
+  const double ll = loglik_of(x, y, W.M[vv], W.M[VC + vv], W.ht[t * VC + vv], inv_lambda);
+  const uint32_t key = make_key(v0 + vv, i, j, h, k);
+  if (ll > best_ll || (ll == best_ll && key < best_key)) { best_ll = ll; best_key = key; }
+}
+
+// One event, all variations, by one warp (see the header of this file).  Returns the winner key in every lane.
+template <int VC, int NBT>
+__device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const RecoCols& ev, const EventHead& h, int V, uint32_t k0,
+                                                 uint32_t k1, const hepf_tth_params_t& P, int lane) {
+  constexpr int LPB = 32 / VC;     // item sub-groups per warp pass
+  constexpr int NP = WarpMem<VC, NBT>::NP;
+  const int vv = lane & (VC - 1), sub = lane / VC;
+  // ---- prologue: nominal objects, kappa*sigma, MET ------------------------------------------------------------------
+  if (lane < 10) {
+    if (lane < 2 + h.n_jet) load_object(ev, h.e, lane, P, &W.obj[lane * 4], W.ks[lane]);
+    else { W.obj[lane * 4] = W.obj[lane * 4 + 1] = W.obj[lane * 4 + 2] = W.obj[lane * 4 + 3] = 0.0; W.ks[lane] = 0.0; }
+  } else if (lane < 12) {
+    W.met[lane - 10] = __ldg((lane == 10 ? ev.met_x : ev.met_y) + h.e);
   }
-  const int64_t S = ev.stride, e = h.e;
-  double dx = 0.0, dy = 0.0, sl[2];
-  V4 lep[2];
-#pragma unroll
-  for (int t = 0; t < 2; t++) {
-    lep[t] = load_v4(ev.lep_px, ev.lep_py, ev.lep_pz, ev.lep_e, t * S + e);
-    const double sc = __fma_rn(__dmul_rn(P.sigma_scale, P.lep_sigma), z[t], 1.0);
-    sl[t] = sc > P.s_min ? sc : P.s_min;
-    const double d = __dadd_rn(sl[t], -1.0);
-    dx = __dadd_rn(dx, __dmul_rn(d, lep[t].x)); dy = __dadd_rn(dy, __dmul_rn(d, lep[t].y));
+  __syncwarp();
+  const int nb = h.n_b, n_pair = nb * (nb - 1) / 2, n_ord = nb * (nb - 1);
+  const uint64_t PK = pair_k_list(nb), PL = pair_l_list(nb);
+  const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
+  const unsigned lt = (1u << lane) - 1u;
+  double best_ll = -CUDART_INF;
+  uint32_t best_key = 0xffffffffu;
+  int qn = 0;                                      // stack height (warp-uniform)
+
+#pragma unroll 1
+  for (int v0 = 0; v0 < V; v0 += VC) {
+    const int nv = min(VC, V - v0);
+    const bool vok = vv < nv;
+    // ---- A: normals -> scales ---------------------------------------------------------------------------------------
+    for (int b0 = 0; b0 < h.nblk; b0 += LPB) {
+      const int blk = b0 + sub;
+      if (vok && blk < h.nblk) {
+        uint32_t x[4];
+        philox4x32_10((uint32_t)h.gidx, (uint32_t)(h.gidx >> 32), (uint32_t)(v0 + vv), 0x54544800u + blk, k0, k1, x);
+        double ze, zo; block_normals(x, ze, zo);
+        W.sc[(2 * blk) * VC + vv] = scale_of(W.ks[2 * blk], ze, P.s_min);
+        W.sc[(2 * blk + 1) * VC + vv] = scale_of(W.ks[2 * blk + 1], zo, P.s_min);
+      }
+    }
+    __syncwarp();
+    // ---- M: MET' = MET - sum_t (s_t - 1) pT_t, summed in slot order ----------------------------------------------------
+#pragma unroll 1
+    for (int c0 = 0; c0 < 2; c0 += LPB) {
+      const int comp = c0 + sub;
+      if (vok && comp < 2) {
+        double acc = 0.0;
+        for (int t = 0; t < 2 + h.n_jet; t++)
+          acc = __dadd_rn(acc, __dmul_rn(__dadd_rn(W.sc[t * VC + vv], -1.0), W.obj[t * 4 + comp]));
+        W.M[comp * VC + vv] = __dadd_rn(W.met[comp], -acc);
+      }
+    }
+    __syncwarp();
+    // ---- B: leg conics (leg 0: l+ with candidate c; leg 1: l- with candidate c, shifted by MET') -------------------------
+    for (int c0 = 0; c0 < 2 * nb; c0 += LPB) {
+      const int comb = c0 + sub;
+      if (vok && comb < 2 * nb) {
+        const int leg = comb >= nb, c = comb - leg * nb;
+        const int ls = leg ? 1 - h.lp_slot : h.lp_slot, js = 2 + ((h.cand >> (4 * c)) & 15);
+        const V4 l = scale_v4(&W.obj[ls * 4], W.sc[ls * VC + vv]), b = scale_v4(&W.obj[js * 4], W.sc[js * VC + vv]);
+        Conic q; double c0_, c1_, c2_;
+        const bool ok = leg_conic(l, b, mt2, mw2, q, c0_, c1_, c2_);
+        if (leg) q = shift_conic(q, W.M[vv], W.M[VC + vv]);
+        const int at = (leg * NBT + c) * VC + vv;
+        W.con[0][at] = ok ? q.a : CUDART_NAN;          // NaN conic -> no roots for any pairing that uses it
+        W.con[1][at] = q.b; W.con[2][at] = q.c; W.con[3][at] = q.d; W.con[4][at] = q.e; W.con[5][at] = q.f;
+      }
+    }
+    // ---- H: Higgs term of every unordered candidate pair ---------------------------------------------------------------
+    for (int p0 = 0; p0 < n_pair; p0 += LPB) {
+      const int p = p0 + sub;
+      if (vok && p < n_pair) {
+        const int kk = (int)(PK >> (4 * p)) & 15, ll = (int)(PL >> (4 * p)) & 15;
+        const int j1 = 2 + ((h.cand >> (4 * kk)) & 15), j2 = 2 + ((h.cand >> (4 * ll)) & 15);
+        const V4 b1 = scale_v4(&W.obj[j1 * 4], W.sc[j1 * VC + vv]), b2 = scale_v4(&W.obj[j2 * 4], W.sc[j2 * VC + vv]);
+        const double t = (mass_of(b1.e + b2.e, b1.x + b2.x, b1.y + b2.y, b1.z + b2.z) - P.m_higgs) * inv_sh;
+        W.ht[pair_index<NBT>(kk, ll) * VC + vv] = -0.5 * (t * t);
+      }
+    }
+    __syncwarp();
+    // ---- C: ordered pairings -> quartic -> roots pushed on the stack; D: pop 32 roots at a time ---------------------------
+    for (int a0 = 0; a0 < n_ord; a0 += LPB) {
+      const int ap = a0 + sub;
+      int mask = 0; uint32_t tag = 0;
+      double xa[2], xb[2];
+      if (vok && ap < n_ord) {
+        const int i = ap / (nb - 1); int j = ap - i * (nb - 1); j += (j >= i);
+        const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
+        const Conic A{W.con[0][a1], W.con[1][a1], W.con[2][a1], W.con[3][a1], W.con[4][a1], W.con[5][a1]};
+        const Conic B{W.con[0][a2], W.con[1][a2], W.con[2][a2], W.con[3][a2], W.con[4][a2], W.con[5][a2]};
+        double g3, g2, g1, g0;
+        resultant(A, B, g3, g2, g1, g0);
+        mask = solve_quartic(g3, g2, g1, g0, xa, xb);
+        if (mask) {
+          double ht; int hh, kk, ll;
+          best_higgs<NBT, VC>(&W.ht[vv], nb, i, j, ht, hh, kk, ll);
+          tag = (uint32_t)vv | (i << 5) | (j << 8) | (hh << 11) | (pair_index<NBT>(kk, ll) << 14);
+        }
+      }
+      // push: Ferrari slots are numbered over the real pairs in the order A+, A-, B+, B-
+      const unsigned bA = __ballot_sync(0xffffffffu, mask & 1), bB = __ballot_sync(0xffffffffu, mask & 2);
+      int at = qn + 2 * (__popc(bA & lt) + __popc(bB & lt));
+      if (mask & 1) { W.qx[at] = xa[0]; W.qtag[at] = tag; W.qx[at + 1] = xa[1]; W.qtag[at + 1] = tag | (1u << 18); at += 2; }
+      if (mask & 2) {
+        const uint32_t s0 = (mask & 1) ? 2u : 0u;
+        W.qx[at] = xb[0]; W.qtag[at] = tag | (s0 << 18); W.qx[at + 1] = xb[1]; W.qtag[at + 1] = tag | ((s0 + 1u) << 18);
+      }
+      qn += 2 * (__popc(bA) + __popc(bB));
+      __syncwarp();
+      while (qn >= 32) {
+        qn -= 32;
+        score_entry<VC, NBT>(W, W.qx[qn + lane], W.qtag[qn + lane], v0, inv_lambda, best_ll, best_key);
+        __syncwarp();
+      }
+    }
+    // the tables are about to be overwritten: score what is left (partial warp)
+    if (qn > 0) {
+      if (lane < qn) score_entry<VC, NBT>(W, W.qx[lane], W.qtag[lane], v0, inv_lambda, best_ll, best_key);
+      qn = 0;
+    }
+    __syncwarp();
   }
+  // ---- argmax over the lanes: max loglik, then the earliest key ---------------------------------------------------------
 #pragma unroll
-  for (int t = 0; t < HEPF_N_JET; t++) {
-    if (t < h.n_jet) {
-      const double E = __ldg(ev.jet_e + t * S + e), px = __ldg(ev.jet_px + t * S + e), py = __ldg(ev.jet_py + t * S + e);
-      const double sigma = __dadd_rn(__ddiv_rn(P.jet_stoch, __dsqrt_rn(E)), P.jet_const);
-      const double sc = __fma_rn(__dmul_rn(P.sigma_scale, sigma), z[2 + t], 1.0);
-      const double s = sc > P.s_min ? sc : P.s_min;
-      const double d = __dadd_rn(s, -1.0);
-      dx = __dadd_rn(dx, __dmul_rn(d, px)); dy = __dadd_rn(dy, __dmul_rn(d, py));
-      const int pos = (h.pos >> (4 * t)) & 15;
-      if (pos < NB_MAX) SM(TH_SCALE + pos) = s;
+  for (int o = 16; o > 0; o >>= 1) {
+    const double oll = __shfl_xor_sync(0xffffffffu, best_ll, o);
+    const uint32_t okey = __shfl_xor_sync(0xffffffffu, best_key, o);
+    if (oll > best_ll || (oll == best_ll && okey < best_key)) { best_ll = oll; best_key = okey; }
+  }
+  return best_key;
+}
+
+// Persistent warps: each warp draws the next group of `epc` consecutive list entries from a global counter; its
+// lanes look at one entry each (index, flags), the entries this instantiation owns are then reconstructed one after the
+// other by the whole warp.  NBT = 4 owns the events with exactly four b candidates (and writes the "nothing to do" key
+// of the non-applicable ones); NBT = 6 owns those with five or six: two launches, each with shared-memory tables sized
+// for its class.
+template <int VC, int NBT, int RW, int MINB>
+__global__ void __launch_bounds__(32 * RW, MINB)
+reco_search_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, int epc, int V, uint32_t k0, uint32_t k1,
+                   hepf_tth_params_t P, uint2* __restrict__ winners, unsigned long long* __restrict__ next_group) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  WarpMem<VC, NBT>& W = reinterpret_cast<WarpMem<VC, NBT>*>(smem_raw)[threadIdx.x >> 5];
+  const int lane = threadIdx.x & 31;
+  const int64_t n_groups = (n_idx + epc - 1) / epc;
+  for (;;) {
+    unsigned long long gq = 0;
+    if (lane == 0) gq = atomicAdd(next_group, 1ull);
+    const int64_t g = (int64_t)__shfl_sync(0xffffffffu, gq, 0);
+    if (g >= n_groups) break;
+    const int64_t kl = g * epc + lane;
+    bool mine = false;
+    if (lane < epc && kl < n_idx) {
+      const EventHead hl = load_head(ev, (int64_t)__ldg(idx + kl));
+      if (!hl.applicable) { if (NBT == 4) winners[kl] = make_uint2(0xffffffffu, 0u); }
+      else mine = (NBT == 4) ? (hl.n_b == 4) : (hl.n_b > 4);
+    }
+    unsigned todo = __ballot_sync(0xffffffffu, mine);
+    while (todo) {
+      const int src = __ffs(todo) - 1; todo &= todo - 1;
+      const int64_t k = g * epc + src;
+      const EventHead h = load_head(ev, (int64_t)__ldg(idx + k));
+      const uint32_t key = search_event<VC, NBT>(W, ev, h, V, k0, k1, P, lane);
+      if (lane == 0) winners[k] = make_uint2(key, key != 0xffffffffu ? 1u : 0u);
+      __syncwarp();
     }
   }
-  Smeared o;
-  o.Mx = __dadd_rn(__ldg(ev.met_x + e), -dx); o.My = __dadd_rn(__ldg(ev.met_y + e), -dy);
-  o.lp = scale_v4(lep[h.lp_slot], sl[h.lp_slot]);
-  o.lm = scale_v4(lep[1 - h.lp_slot], sl[1 - h.lp_slot]);
-  return o;
 }
 
-__device__ __forceinline__ V4 smeared_cand(const RecoCols& ev, const EventHead& h, int c, const double* sm) {
-  const int slot = (h.cand >> (4 * c)) & 15;
-  const V4 nom = load_v4(ev.jet_px, ev.jet_py, ev.jet_pz, ev.jet_e, slot * ev.stride + h.e);
-  return scale_v4(nom, SM(TH_SCALE + c));
-}
-
-struct Cand { double ll; double x; int v, a, h; };
-
-__device__ __forceinline__ unsigned long long ordered_key(double v) {   // monotone map double -> uint64
-  const long long b = __double_as_longlong(v);
-  return (b < 0) ? ~(unsigned long long)b : ((unsigned long long)b | 0x8000000000000000ull);
-}
-
-__global__ void __launch_bounds__(RECO_THREADS)
-reco_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, int V, uint32_t k0, uint32_t k1,
-            hepf_tth_params_t P, hepf_best_t* __restrict__ out) {
-  extern __shared__ double sm[];
-  __shared__ unsigned long long s_key[RECO_THREADS];
-  __shared__ unsigned long long s_flat[RECO_THREADS];
-  const int tid = threadIdx.x;
-  const int lpe = V < RECO_THREADS ? V : RECO_THREADS;   // lanes per event
-  const int epb = RECO_THREADS / lpe;                    // events per block
-  const int slot = tid / lpe, v_first = tid - slot * lpe;
-  const int64_t k = (int64_t)blockIdx.x * epb + slot;    // position in idx
-  const bool live = slot < epb && k < n_idx;
-  if (tid < epb) { s_key[tid] = 0ull; s_flat[tid] = ~0ull; }
-  __syncthreads();
-
-  EventHead h{};
-  Cand best{-CUDART_INF, 0.0, -1, -1, -1};
-  const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, inv_lambda = 1.0 / P.lambda_nu, inv_sh = 1.0 / P.sigma_higgs;
-  if (live) {
-    h = load_head(ev, (int64_t)__ldg(idx + k));
-    if (h.applicable) {
-      const int nb = h.n_b;
-      for (int v = v_first; v < V; v += RECO_THREADS) {
-        const Smeared S = smear_variation(ev, h, v, k0, k1, P, sm);
-        // ---- per-variation tables: leg-2 conics (shifted by MET') and Higgs terms of all candidate pairs --------
-        for (int j = 0; j < nb; j++) {
-          const V4 bj = smeared_cand(ev, h, j, sm);
-          Conic q; double c0, c1, c2;
-          const bool ok = leg_conic(S.lm, bj, mt2, mw2, q, c0, c1, c2);
-          const Conic s2 = shift_conic(q, S.Mx, S.My);
-          SM(TH_CONIC2 + 6 * j + 0) = ok ? s2.a : CUDART_NAN;   // NaN conic -> no roots for this pairing
-          SM(TH_CONIC2 + 6 * j + 1) = s2.b; SM(TH_CONIC2 + 6 * j + 2) = s2.c;
-          SM(TH_CONIC2 + 6 * j + 3) = s2.d; SM(TH_CONIC2 + 6 * j + 4) = s2.e; SM(TH_CONIC2 + 6 * j + 5) = s2.f;
-          for (int l = j + 1; l < nb; l++) {
-            const V4 bl = smeared_cand(ev, h, l, sm);
-            const double mbb = mass_of(bj.e + bl.e, bj.x + bl.x, bj.y + bl.y, bj.z + bl.z);
-            const double t = (mbb - P.m_higgs) * inv_sh;
-            SM(TH_HT + tri(j, l)) = -0.5 * (t * t);
-          }
-        }
-        // ---- ordered pairings ---------------------------------------------------------------------------------------
-        for (int i = 0; i < nb; i++) {
-          const V4 bi = smeared_cand(ev, h, i, sm);
-          Conic k1c; double c0, c1, c2;
-          const bool ok1 = leg_conic(S.lp, bi, mt2, mw2, k1c, c0, c1, c2);
-          if (!ok1) k1c.a = CUDART_NAN;
-          for (int j = 0; j < nb; j++) {
-            if (j == i) continue;
-            const Conic k2c{SM(TH_CONIC2 + 6 * j + 0), SM(TH_CONIC2 + 6 * j + 1), SM(TH_CONIC2 + 6 * j + 2),
-                            SM(TH_CONIC2 + 6 * j + 3), SM(TH_CONIC2 + 6 * j + 4), SM(TH_CONIC2 + 6 * j + 5)};
-            const Resultant R = resultant(k1c, k2c);
-            double x[4];
-            const int nr = solve_quartic(R.g3, R.g2, R.g1, R.g0, x);
-            if (nr == 0) continue;
-            // best Higgs pair among the candidates not used by (i, j), lexicographic order, first maximum
-            double ht = -CUDART_INF; int hbest = 0, hcount = 0;
-            for (int kk = 0; kk < nb; kk++) for (int l = kk + 1; l < nb; l++) {
-              if (kk == i || kk == j || l == i || l == j) continue;
-              const double t = SM(TH_HT + tri(kk, l));
-              if (t > ht) { ht = t; hbest = hcount; }
-              hcount++;
-            }
-            for (int rr = 0; rr < nr; rr++) {
-              double xx = x[rr], yy; refine_xy(R, k1c, k2c, xx, yy);
-              const double qx = S.Mx - xx, qy = S.My - yy;
-              const double ptn = sqrt(xx * xx + yy * yy), ptb = sqrt(qx * qx + qy * qy);
-              const double ll = ht + (log(ptn * ptb) - (ptn + ptb) * inv_lambda);
-              if (ll > best.ll) { best.ll = ll; best.x = xx; best.v = v; best.a = i * nb + j; best.h = hbest; }
-            }
-          }
-        }
+// One thread per selected event: re-derive the winner in full and write the record.
+__global__ void __launch_bounds__(128)
+reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, uint32_t k0, uint32_t k1,
+                     hepf_tth_params_t P, const uint2* __restrict__ winners, hepf_best_t* __restrict__ out) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n_idx) return;
+  const EventHead h = load_head(ev, (int64_t)__ldg(idx + k));
+  const uint2 w = winners[k];
+  hepf_best_t* o = out + k;
+  if (!h.applicable || !w.y) {
+    const double n = CUDART_NAN;
+    o->nu[0] = o->nu[1] = o->nu[2] = o->nubar[0] = o->nubar[1] = o->nubar[2] = n;
+    o->m_top = o->m_antitop = o->m_wplus = o->m_wminus = o->m_higgs = o->loglik = n;
+    o->variation = o->jet_b = o->jet_bbar = o->jet_h1 = o->jet_h2 = o->root = -1;
+    o->status = h.status; o->event = (uint32_t)h.e;
+    return;
+  }
+  const int v = (int)(w.x >> 11), a6 = (w.x >> 5) & 63, i = a6 / 6, j = a6 - 6 * i, hsel = (w.x >> 2) & 7, ksel = w.x & 3;
+  const int nb = h.n_b;
+  const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
+  // smear this variation
+  double obj[10][4], sc[10];
+  double ax = 0.0, ay = 0.0;
+  for (int blk = 0; blk < h.nblk; blk++) {
+    uint32_t x[4];
+    philox4x32_10((uint32_t)h.gidx, (uint32_t)(h.gidx >> 32), (uint32_t)v, 0x54544800u + blk, k0, k1, x);
+    double z[2]; block_normals(x, z[0], z[1]);
+    for (int u = 0; u < 2; u++) {
+      const int t = 2 * blk + u;
+      double ks = 0.0;
+      if (t < 2 + h.n_jet) load_object(ev, h.e, t, P, obj[t], ks);
+      else obj[t][0] = obj[t][1] = obj[t][2] = obj[t][3] = 0.0;
+      sc[t] = scale_of(ks, z[u], P.s_min);
+      if (t < 2 + h.n_jet) {
+        const double d = __dadd_rn(sc[t], -1.0);
+        ax = __dadd_rn(ax, __dmul_rn(d, obj[t][0])); ay = __dadd_rn(ay, __dmul_rn(d, obj[t][1]));
       }
     }
   }
-  // ---- argmax over the threads of one event: max loglik, then lowest (variation, pairing) ----------------------
-  const bool have = live && best.v >= 0;
-  const unsigned long long key = have ? ordered_key(best.ll) : 0ull;
-  const unsigned long long flat = have ? (((unsigned long long)best.v << 8) | (unsigned long long)best.a) : ~0ull;
-  if (have) atomicMax(&s_key[slot], key);
-  __syncthreads();
-  if (have && key == s_key[slot]) atomicMin(&s_flat[slot], flat);
-  __syncthreads();
-  if (!live) return;
-  hepf_best_t* o = out + k;
-  if (s_key[slot] == 0ull) {                     // no thread of this event found a solution
-    if (v_first == 0) {
-      const double n = CUDART_NAN;
-      o->nu[0] = o->nu[1] = o->nu[2] = o->nubar[0] = o->nubar[1] = o->nubar[2] = n;
-      o->m_top = o->m_antitop = o->m_wplus = o->m_wminus = o->m_higgs = o->loglik = n;
-      o->variation = o->jet_b = o->jet_bbar = o->jet_h1 = o->jet_h2 = o->root = -1;
-      o->status = h.status; o->event = (uint32_t)h.e;
-    }
-    return;
+  const double Mx = __dadd_rn(__ldg(ev.met_x + h.e), -ax), My = __dadd_rn(__ldg(ev.met_y + h.e), -ay);
+  const int lps = h.lp_slot, lms = 1 - h.lp_slot;
+  const int si = (h.cand >> (4 * i)) & 15, sj = (h.cand >> (4 * j)) & 15;
+  const V4 lp = scale_v4(obj[lps], sc[lps]), lm = scale_v4(obj[lms], sc[lms]);
+  const V4 bi = scale_v4(obj[2 + si], sc[2 + si]), bj = scale_v4(obj[2 + sj], sc[2 + sj]);
+  Conic A, q2; double c0, c1, c2, e0, e1, e2;
+  leg_conic(lp, bi, mt2, mw2, A, c0, c1, c2);
+  leg_conic(lm, bj, mt2, mw2, q2, e0, e1, e2);
+  const Conic B = shift_conic(q2, Mx, My);
+  double g3, g2, g1, g0, xa[2] = {0, 0}, xb[2] = {0, 0};
+  resultant(A, B, g3, g2, g1, g0);
+  const int mask = solve_quartic(g3, g2, g1, g0, xa, xb);
+  double xs[4], ys[4]; int nr = 0;
+  if (mask & 1) { xs[0] = xa[0]; xs[1] = xa[1]; nr = 2; }
+  if (mask & 2) { xs[nr] = xb[0]; xs[nr + 1] = xb[1]; nr += 2; }
+  for (int r = 0; r < nr; r++) refine_xy(A, B, xs[r], ys[r]);
+  const int rs = ksel < nr ? ksel : 0;
+  const double xx = nr ? xs[rs] : CUDART_NAN, yy = nr ? ys[rs] : CUDART_NAN;
+  int rank = 0;
+  for (int r = 0; r < nr; r++) rank += (xs[r] < xx) || (xs[r] == xx && r < rs);
+  // Higgs pair hsel among the candidates not used by (i, j)
+  int hk = 0, hl = 1, hc = 0;
+  for (int kk = 0; kk < nb; kk++) for (int l = kk + 1; l < nb; l++) {
+    if (kk == i || kk == j || l == i || l == j) continue;
+    if (hc == hsel) { hk = kk; hl = l; }
+    hc++;
   }
-  if (!(have && key == s_key[slot] && flat == s_flat[slot])) return;
-  // ---- the winner re-derives its solution in full and writes the record ---------------------------------------------
-  {
-    const int nb = h.n_b, i = best.a / nb, j = best.a - i * nb;
-    const Smeared S = smear_variation(ev, h, best.v, k0, k1, P, sm);
-    const V4 bi = smeared_cand(ev, h, i, sm), bj = smeared_cand(ev, h, j, sm);
-    Conic k1c, q2; double c0, c1, c2, e0, e1, e2;
-    leg_conic(S.lp, bi, mt2, mw2, k1c, c0, c1, c2);
-    leg_conic(S.lm, bj, mt2, mw2, q2, e0, e1, e2);
-    const Conic k2c = shift_conic(q2, S.Mx, S.My);
-    const Resultant R = resultant(k1c, k2c);
-    double x[4];
-    const int nr = solve_quartic(R.g3, R.g2, R.g1, R.g0, x);
-    // polish every root as the hot loop did; the winner is the recomputed root closest to the remembered one,
-    // its rank is its position among the real roots in ascending order
-    double ys[4];
-    for (int r = 0; r < nr; r++) refine_xy(R, k1c, k2c, x[r], ys[r]);
-    int rsel = 0; double dmin = CUDART_INF;
-    for (int r = 0; r < nr; r++) { const double d = fabs(x[r] - best.x); if (d < dmin) { dmin = d; rsel = r; } }
-    const double xx = (nr > 0) ? x[rsel] : best.x;
-    const double yy = (nr > 0) ? ys[rsel] : CUDART_NAN;
-    int rank = 0;
-    for (int r = 0; r < nr; r++) rank += (x[r] < xx) || (x[r] == xx && r < rsel);
-    const double pz = c0 + c1 * xx + c2 * yy;
-    const double qx = S.Mx - xx, qy = S.My - yy, qz = e0 + e1 * qx + e2 * qy;
-    const double en = sqrt(xx * xx + yy * yy + pz * pz), eb = sqrt(qx * qx + qy * qy + qz * qz);
-    // Higgs pair index -> candidate positions
-    int hk = -1, hl = -1, hcount = 0;
-    for (int kk = 0; kk < nb; kk++) for (int l = kk + 1; l < nb; l++) {
-      if (kk == i || kk == j || l == i || l == j) continue;
-      if (hcount == best.h) { hk = kk; hl = l; }
-      hcount++;
-    }
-    const V4 h1 = smeared_cand(ev, h, hk, sm), h2 = smeared_cand(ev, h, hl, sm);
-    const double mbb = mass_of(h1.e + h2.e, h1.x + h2.x, h1.y + h2.y, h1.z + h2.z);
-    const double ptn = sqrt(xx * xx + yy * yy), ptb = sqrt(qx * qx + qy * qy);
-    const double t = (mbb - P.m_higgs) * inv_sh;
-    o->nu[0] = xx; o->nu[1] = yy; o->nu[2] = pz;
-    o->nubar[0] = qx; o->nubar[1] = qy; o->nubar[2] = qz;
-    o->m_wplus = mass_of(S.lp.e + en, S.lp.x + xx, S.lp.y + yy, S.lp.z + pz);
-    o->m_top = mass_of(S.lp.e + en + bi.e, S.lp.x + xx + bi.x, S.lp.y + yy + bi.y, S.lp.z + pz + bi.z);
-    o->m_wminus = mass_of(S.lm.e + eb, S.lm.x + qx, S.lm.y + qy, S.lm.z + qz);
-    o->m_antitop = mass_of(S.lm.e + eb + bj.e, S.lm.x + qx + bj.x, S.lm.y + qy + bj.y, S.lm.z + qz + bj.z);
-    o->m_higgs = mbb;
-    o->loglik = -0.5 * (t * t) + (log(ptn * ptb) - (ptn + ptb) * inv_lambda);
-    o->variation = best.v;
-    o->jet_b = (h.cand >> (4 * i)) & 15; o->jet_bbar = (h.cand >> (4 * j)) & 15;
-    o->jet_h1 = (h.cand >> (4 * hk)) & 15; o->jet_h2 = (h.cand >> (4 * hl)) & 15;
-    o->root = rank;
-    o->status = h.status | 1u; o->event = (uint32_t)h.e;
+  const int sh1 = (h.cand >> (4 * hk)) & 15, sh2 = (h.cand >> (4 * hl)) & 15;
+  const V4 h1 = scale_v4(obj[2 + sh1], sc[2 + sh1]), h2 = scale_v4(obj[2 + sh2], sc[2 + sh2]);
+  const double mbb = mass_of(h1.e + h2.e, h1.x + h2.x, h1.y + h2.y, h1.z + h2.z);
+  const double t = (mbb - P.m_higgs) * inv_sh, ht = -0.5 * (t * t);
+  const double pz = fma(c2, yy, fma(c1, xx, c0));
+  const double qx = Mx - xx, qy = My - yy, qz = fma(e2, qy, fma(e1, qx, e0));
+  const double en = sqrt_fast(fma(xx, xx, fma(yy, yy, pz * pz))), eb = sqrt_fast(fma(qx, qx, fma(qy, qy, qz * qz)));
+  o->nu[0] = xx; o->nu[1] = yy; o->nu[2] = pz;
+  o->nubar[0] = qx; o->nubar[1] = qy; o->nubar[2] = qz;
+  o->m_wplus = mass_of(lp.e + en, lp.x + xx, lp.y + yy, lp.z + pz);
+  o->m_top = mass_of(lp.e + en + bi.e, lp.x + xx + bi.x, lp.y + yy + bi.y, lp.z + pz + bi.z);
+  o->m_wminus = mass_of(lm.e + eb, lm.x + qx, lm.y + qy, lm.z + qz);
+  o->m_antitop = mass_of(lm.e + eb + bj.e, lm.x + qx + bj.x, lm.y + qy + bj.y, lm.z + qz + bj.z);
+  o->m_higgs = mbb;
+  o->loglik = loglik_of(xx, yy, Mx, My, ht, inv_lambda);
+  o->variation = v;
+  o->jet_b = si; o->jet_bbar = sj; o->jet_h1 = sh1; o->jet_h2 = sh2;
+  o->root = rank;
+  o->status = h.status | 1u; o->event = (uint32_t)h.e;
+}
+
+// HEPF_RECO_CFG (8, 161, 163, 164) overrides the launch shape; for tuning experiments only
+static int reco_tuning() {
+  static const int v = [] { const char* e = getenv("HEPF_RECO_CFG"); return e ? atoi(e) : 0; }();
+  return v;
+}
+
+template <int VC, int NBT, int RW, int MINB>
+static int launch_search(const RecoCols& cols, const uint32_t* idx, int64_t n_idx, int V, uint64_t seed,
+                         const hepf_tth_params_t& P, uint2* winners, unsigned long long* counter, cudaStream_t stream) {
+  const size_t smem = sizeof(WarpMem<VC, NBT>) * RW;
+  auto kern = reco_search_kernel<VC, NBT, RW, MINB>;
+  static thread_local int blocks_per_sm = 0, sms = 0;
+  if (!blocks_per_sm) {
+    int dev = 0;
+    HEPF_CUDA_TRY(cudaGetDevice(&dev));
+    HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    HEPF_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    HEPF_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    HEPF_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, 32 * RW, smem));
+    if (blocks_per_sm < 1) { set_error("hepf_reconstruct_tth: search kernel does not fit on an SM"); return HEPF_ERR_CUDA; }
   }
+  // persistent grid; groups of up to 8 list entries, fewer when the list is short
+  const int64_t max_warps = (int64_t)sms * blocks_per_sm * RW;
+  int epc = 8;
+  while (epc > 1 && (n_idx + epc - 1) / epc < 8 * max_warps) epc >>= 1;
+  const int64_t n_groups = (n_idx + epc - 1) / epc;
+  const int64_t want = (n_groups + RW - 1) / RW, cap = (int64_t)sms * blocks_per_sm;
+  const unsigned grid = (unsigned)(want < cap ? want : cap);
+  kern<<<grid, 32 * RW, smem, stream>>>(cols, idx, n_idx, epc, V, (uint32_t)seed, (uint32_t)(seed >> 32), P, winners, counter);
+  count_launch();
+  HEPF_CUDA_TRY(cudaGetLastError());
+  return HEPF_OK;
+}
+
+// both candidate-count classes: n_b = 4 (tables for 4 candidates, more warps per SM) and n_b = 5, 6
+template <int VC, int RW, int MINB4, int MINB6>
+static int launch_search_both(const RecoCols& cols, const uint32_t* idx, int64_t n_idx, int V, uint64_t seed,
+                              const hepf_tth_params_t& P, uint2* winners, cudaStream_t stream) {
+  unsigned long long* counters = reinterpret_cast<unsigned long long*>(winners + n_idx);   // two group counters
+  HEPF_CUDA_TRY(cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), stream));
+  const int rc = launch_search<VC, 4, RW, MINB4>(cols, idx, n_idx, V, seed, P, winners, counters, stream);
+  if (rc != HEPF_OK) return rc;
+  return launch_search<VC, 6, RW, MINB6>(cols, idx, n_idx, V, seed, P, winners, counters + 1, stream);
 }
 
 }  // namespace hepf
@@ -431,41 +722,45 @@ reco_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, int V,
 using namespace hepf;
 
 extern "C" size_t hepf_reconstruct_workspace_bytes(int64_t n_idx, int32_t n_variations) {
-  (void)n_idx; (void)n_variations;
-  return 0;   // all intermediate state lives in registers and shared memory
+  (void)n_variations;
+  if (n_idx < 0) return 0;
+  return (size_t)(n_idx > 0 ? n_idx : 1) * sizeof(uint2) + 16;   // one winner key per listed event + two work counters
 }
 
 extern "C" int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
                                     uint64_t seed, const hepf_tth_params_t* host_params, hepf_best_t* out_best, void* ws,
                                     size_t ws_bytes, void* stream_) {
-  (void)ws; (void)ws_bytes;
   cudaStream_t stream = (cudaStream_t)stream_;
   int rc = check_events(events);
   if (rc != HEPF_OK) return rc;
-  if (n_idx < 0 || n_variations < 1 || n_variations > (1 << 23)) {
-    set_error("hepf_reconstruct_tth: need n_idx >= 0 and 1 <= n_variations <= 2^23"); return HEPF_ERR_ARG;
+  if (n_idx < 0 || n_variations < 1 || n_variations > (1 << 21)) {
+    set_error("hepf_reconstruct_tth: need n_idx >= 0 and 1 <= n_variations <= 2^21"); return HEPF_ERR_ARG;
   }
   if (n_idx == 0) return HEPF_OK;
   if (!idx || !aligned(idx, 4) || !out_best || !aligned(out_best, 16)) {
     set_error("hepf_reconstruct_tth: idx/out_best NULL or misaligned"); return HEPF_ERR_ARG;
   }
+  if (!ws || !aligned(ws, 8) || ws_bytes < hepf_reconstruct_workspace_bytes(n_idx, n_variations)) {
+    set_error("hepf_reconstruct_tth: workspace too small or misaligned (%zu < %zu)", ws_bytes,
+              hepf_reconstruct_workspace_bytes(n_idx, n_variations));
+    return HEPF_ERR_CAPACITY;
+  }
   hepf_tth_params_t P;
   if (host_params) P = *host_params; else hepf_default_params(&P);
-  RecoCols cols{events->lep_px, events->lep_py, events->lep_pz, events->lep_e, events->jet_px, events->jet_py,
-                events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags,
-                events->n_events, events->stride, events->event_base};
-  const int lpe = n_variations < RECO_THREADS ? n_variations : RECO_THREADS;
-  const int epb = RECO_THREADS / lpe;
-  const int64_t blocks = (n_idx + epb - 1) / epb;
-  if (blocks > 0x7fffffffll) { set_error("hepf_reconstruct_tth: too many blocks"); return HEPF_ERR_ARG; }
-  const size_t smem = (size_t)TH_DOUBLES * RECO_THREADS * sizeof(double);
-  static thread_local bool attr_set = false;
-  if (!attr_set) {
-    HEPF_CUDA_TRY(cudaFuncSetAttribute(reco_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set = true;
-  }
-  reco_kernel<<<(unsigned)blocks, RECO_THREADS, smem, stream>>>(cols, idx, n_idx, n_variations, (uint32_t)seed,
-                                                               (uint32_t)(seed >> 32), P, out_best);
+  const RecoCols cols{events->lep_px, events->lep_py, events->lep_pz, events->lep_e, events->jet_px, events->jet_py,
+                      events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags,
+                      events->n_events, events->stride, events->event_base};
+  uint2* winners = reinterpret_cast<uint2*>(ws);
+  const int cfg = reco_tuning();
+  if (n_variations <= 8 || cfg == 8) rc = launch_search_both<8, 2, 12, 10>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  else if (cfg == 161) rc = launch_search_both<16, 1, 20, 14>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  else if (cfg == 163) rc = launch_search_both<16, 2, 8, 6>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  else if (cfg == 164) rc = launch_search_both<16, 4, 5, 3>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  else rc = launch_search_both<16, 2, 10, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  if (rc != HEPF_OK) return rc;
+  const int64_t fblocks = (n_idx + 127) / 128;
+  reco_finalize_kernel<<<(unsigned)fblocks, 128, 0, stream>>>(cols, idx, n_idx, (uint32_t)seed, (uint32_t)(seed >> 32), P,
+                                                             winners, out_best);
   count_launch();
   HEPF_CUDA_TRY(cudaGetLastError());
   return HEPF_OK;
