@@ -30,9 +30,13 @@ METRIC = "smeared ttH reconstructions/sec (event x assignment x variation)"
 UNIT = "reconstructions/s"
 # FP64 roof of one B200 from the guide's unit counts: 148 SMs x 64 FP64 FMA lanes/clk x 2 flop x clocks.max.sm
 FP64_LANES_PER_SM = 64
-# Algorithmic FP64 work of one solve (flop, FMA = 2): measured thread-level
-# dadd + dmul + 2 dfma of reco_kernel divided by the solves of the profiled launch (profiles/r01_*).
-FLOP_PER_SOLVE = {"cfg1": 3100.0, "cfg2": 3100.0, "cfg3": 3100.0, "cfg4": 3100.0}
+# Algorithmic FP64 work of one solve: the search kernel's own predicated-on thread-level FP64 instruction counts per
+# solve (idle lanes and divergence waste do not count), from the committed ncu capture of this build
+# (profiles/r01c_reco_search.md): DADD + DMUL + DFMA lane-ops, and flop with FMA = 2.  DESIGN.md section 7.
+FP64_OPS_PER_SOLVE = {"dadd": 36.1, "dmul": 93.7, "dfma": 171.5}
+LANE_OPS_PER_SOLVE = sum(FP64_OPS_PER_SOLVE.values())
+FLOP_PER_SOLVE = FP64_OPS_PER_SOLVE["dadd"] + FP64_OPS_PER_SOLVE["dmul"] + 2.0 * FP64_OPS_PER_SOLVE["dfma"]
+DRAM_BYTES_PER_LAUNCH = 274.6e6   # ncu dram__bytes_read.sum + dram__bytes_write.sum of the search kernel (same profile)
 
 
 def solves_of(store, idx, n_variations: int) -> int:
@@ -91,10 +95,10 @@ def cpu_oracle_rate(store, idx, n_variations, seed, target_s=15.0):
     """Time the oracle, as it stands, on a bounded sample of the same workload on the host cores."""
     import oracle
     cores = os.cpu_count() or 1
-    probe = idx[:64]
+    probe = idx[:2048]
     t0 = time.perf_counter(); oracle.reconstruct_tth(store, probe, n_variations, seed, n_threads=cores)
     dt = max(time.perf_counter() - t0, 1e-3)
-    m = int(min(len(idx), max(64, 64 * target_s / dt)))
+    m = int(min(len(idx), max(2048, 2048 * target_s / dt)))
     sample = idx[:m]
     t0 = time.perf_counter()
     oracle.select(store, hs.CHAIN_BASE)            # the oracle's selection of the whole batch is part of a step
@@ -206,11 +210,16 @@ def main():
     hepf.launch_count(reset=True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     mids = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    binding.timing_enable(True)
+    k_search, k_final, k_sel = [], [], []
     e0.record(stream)
     for s in range(args.steps):
         step(mids[s])
+        # device time of each kernel of this step, from events the library records on the stream around its launches
+        k_search.append(binding.timing_ms(3, 4)); k_final.append(binding.timing_ms(5, 6)); k_sel.append(binding.timing_ms(0, 2))
     e1.record(stream)
     torch.cuda.synchronize()
+    binding.timing_enable(False)
     launches = hepf.launch_count()
     clocks = sampler.stop()
     ms_total = e0.elapsed_time(e1)
@@ -264,13 +273,19 @@ def main():
     p0.record(stream); binding.fp64_peak_probe(sms * 8, 256, per_thread, sink, stream); p1.record(stream)
     torch.cuda.synchronize()
     fma_peak = 2.0 * sms * 8 * 256 * per_thread / (p0.elapsed_time(p1) * 1e-3) / 1e12
-    achieved = FLOP_PER_SOLVE[args.workload] * n_solves / (ms_reco * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "reco_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": None,
-                "peak_source": f"{sms} SMs x {FP64_LANES_PER_SM} FP64 FMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md)",
+    ms_search = float(np.mean(k_search))
+    achieved = FLOP_PER_SOLVE * n_solves / (ms_search * 1e-3) / 1e12
+    lane_rate = LANE_OPS_PER_SOLVE * n_solves / (ms_search * 1e-3)
+    lane_peak = sms * FP64_LANES_PER_SM * sm_max * 1e6
+    roofline = {"bound": "alu", "kernel": "reco_search_kernel<16,4>", "achieved": achieved, "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": DRAM_BYTES_PER_LAUNCH,
+                "peak_source": f"{sms} SMs x {FP64_LANES_PER_SM} FP64 FMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md section 6.2)",
                 "dfma_chain_measured_tflops": fma_peak, "frac_of_measured_dfma": achieved / fma_peak,
-                "flop_per_solve": FLOP_PER_SOLVE[args.workload], "kernel_ms": ms_reco,
-                "kernel_share_of_step": ms_reco / ms_per_step}
+                "fp64_lane_ops_per_solve": LANE_OPS_PER_SOLVE, "flop_per_solve": FLOP_PER_SOLVE,
+                "fp64_pipe_frac": lane_rate / lane_peak, "kernel_ms": ms_search,
+                "kernel_share_of_step": ms_search / ms_per_step,
+                "other_kernels_ms": {"select_eval+scatter": float(np.mean(k_sel)), "reco_finalize": float(np.mean(k_final)),
+                                     "hepf_reconstruct_tth_call": ms_reco}}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",

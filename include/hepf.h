@@ -153,6 +153,14 @@ int64_t hepf_launch_count(int reset);
  * `fma_per_thread` dependent-chain-of-8 DFMAs per thread over blocks x threads; writes a checksum to `sink`. */
 int hepf_fp64_peak_probe(int blocks, int threads, int64_t fma_per_thread, double* sink, void* stream);
 
+/* Per-kernel device timing for bench.py's roofline: when enabled (per host thread) the library records a CUDA event on
+ * the call's stream before and after each of its kernels.  Slots: 0 select start | 1 after select_eval | 2 after
+ * select_scatter | 3 reconstruct start | 4 after the n_b = 4 search kernel | 5 after the n_b = 5,6 search kernel |
+ * 6 after the finalize kernel.  hepf_timing_ms waits for the `to` event and returns the elapsed milliseconds of the
+ * LAST call that recorded both (negative if unavailable). */
+int hepf_timing_enable(int on);
+double hepf_timing_ms(int from_slot, int to_slot);
+
 const char* hepf_last_error(void);
 const char* hepf_version(void);
 

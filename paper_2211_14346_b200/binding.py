@@ -76,6 +76,9 @@ def load():
         L.hepf_tth_host.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_int32, C.c_uint64,
                                     C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_size_t, C.c_void_p]
+        L.hepf_timing_enable.argtypes = [C.c_int]
+        L.hepf_timing_ms.restype = C.c_double
+        L.hepf_timing_ms.argtypes = [C.c_int, C.c_int]
         L.hepf_fp64_peak_probe.argtypes = [C.c_int, C.c_int, C.c_int64, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
@@ -236,3 +239,12 @@ def tth_host(store, chain, n_variations: int, seed: int, params: Params | None =
 def fp64_peak_probe(blocks: int, threads: int, fma_per_thread: int, sink, stream=None):
     rc = load().hepf_fp64_peak_probe(blocks, threads, fma_per_thread, sink.data_ptr(), _stream_ptr(stream))
     _check(rc, "hepf_fp64_peak_probe")
+
+
+def timing_enable(on: bool = True):
+    load().hepf_timing_enable(int(on))
+
+
+def timing_ms(from_slot: int, to_slot: int) -> float:
+    """Elapsed device milliseconds between two of the library's timing slots (see include/hepf.h)."""
+    return float(load().hepf_timing_ms(from_slot, to_slot))

@@ -20,6 +20,14 @@ int cuda_fail(cudaError_t e, const char* what) {
 }
 void count_launch(int n) { g_launches += n; }
 
+static thread_local bool g_timing = false;
+static thread_local cudaEvent_t g_ev[T_SLOTS] = {};
+void timing_mark(int slot, cudaStream_t stream) {
+  if (!g_timing || slot < 0 || slot >= T_SLOTS) return;
+  if (!g_ev[slot] && cudaEventCreate(&g_ev[slot]) != cudaSuccess) return;
+  cudaEventRecord(g_ev[slot], stream);
+}
+
 int check_events(const hepf_events_t* ev) {
   if (!ev) { set_error("events view is NULL"); return HEPF_ERR_ARG; }
   if (ev->n_events < 0 || ev->stride < ev->n_events || (ev->stride & 1)) {
@@ -53,6 +61,14 @@ __global__ void fp64_peak_kernel(int64_t iters, double* sink) {
 
 using namespace hepf;
 
+extern "C" int hepf_timing_enable(int on) { g_timing = on != 0; return HEPF_OK; }
+extern "C" double hepf_timing_ms(int from_slot, int to_slot) {
+  if (from_slot < 0 || to_slot < 0 || from_slot >= T_SLOTS || to_slot >= T_SLOTS || !g_ev[from_slot] || !g_ev[to_slot]) return -1.0;
+  if (cudaEventSynchronize(g_ev[to_slot]) != cudaSuccess) return -1.0;
+  float ms = -1.0f;
+  if (cudaEventElapsedTime(&ms, g_ev[from_slot], g_ev[to_slot]) != cudaSuccess) return -1.0;
+  return (double)ms;
+}
 extern "C" const char* hepf_last_error(void) { return g_err; }
 extern "C" const char* hepf_version(void) { return "hepf 0.1 (sm_100a)"; }
 extern "C" int64_t hepf_launch_count(int reset) {

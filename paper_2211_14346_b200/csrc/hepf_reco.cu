@@ -712,9 +712,13 @@ static int launch_search_both(const RecoCols& cols, const uint32_t* idx, int64_t
                               const hepf_tth_params_t& P, uint2* winners, cudaStream_t stream) {
   unsigned long long* counters = reinterpret_cast<unsigned long long*>(winners + n_idx);   // two group counters
   HEPF_CUDA_TRY(cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), stream));
-  const int rc = launch_search<VC, 4, RW, MINB4>(cols, idx, n_idx, V, seed, P, winners, counters, stream);
+  timing_mark(T_RECO0, stream);
+  int rc = launch_search<VC, 4, RW, MINB4>(cols, idx, n_idx, V, seed, P, winners, counters, stream);
+  timing_mark(T_RECO1, stream);
   if (rc != HEPF_OK) return rc;
-  return launch_search<VC, 6, RW, MINB6>(cols, idx, n_idx, V, seed, P, winners, counters + 1, stream);
+  rc = launch_search<VC, 6, RW, MINB6>(cols, idx, n_idx, V, seed, P, winners, counters + 1, stream);
+  timing_mark(T_RECO2, stream);
+  return rc;
 }
 
 }  // namespace hepf
@@ -762,6 +766,7 @@ extern "C" int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t*
   reco_finalize_kernel<<<(unsigned)fblocks, 128, 0, stream>>>(cols, idx, n_idx, (uint32_t)seed, (uint32_t)(seed >> 32), P,
                                                              winners, out_best);
   count_launch();
+  timing_mark(T_RECO3, stream);
   HEPF_CUDA_TRY(cudaGetLastError());
   return HEPF_OK;
 }

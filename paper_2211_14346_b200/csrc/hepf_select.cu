@@ -237,12 +237,15 @@ extern "C" int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_c
                                                       align_up((size_t)(n_tiles + 1) * SEL_WARPS * sizeof(uint2), 256));
   SelCols cols{events->lep_pt, events->lep_eta, events->jet_pt, events->jet_eta, events->met, events->mll,
                events->flags, n, events->stride};
+  timing_mark(T_SEL0, stream);
   select_eval_kernel<<<grid, SEL_THREADS, 0, stream>>>(cols, chain, n_tiles, tpb, masks, block_count,
                                                        (n_cuts > 0) ? reinterpret_cast<unsigned long long*>(out_cutflow) : nullptr);
   count_launch();
   HEPF_CUDA_TRY(cudaGetLastError());
+  timing_mark(T_SEL1, stream);
   select_scatter_kernel<<<grid, SEL_THREADS, 0, stream>>>(n_tiles, tpb, masks, block_count, out_idx, out_count);
   count_launch();
+  timing_mark(T_SEL2, stream);
   HEPF_CUDA_TRY(cudaGetLastError());
   return HEPF_OK;
 }
