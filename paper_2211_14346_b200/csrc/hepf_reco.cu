@@ -96,27 +96,44 @@ __device__ __forceinline__ double mass_of(double e, double x, double y, double z
   return sqrt_fast(m2 > 0.0 ? m2 : 0.0);
 }
 
-// Leg conic of (lepton l, b-jet b): neutrino p_z = c0 + c1 p_x + c2 p_y and the conic in (p_x, p_y).
-__device__ __forceinline__ bool leg_conic(const V4& l, const V4& b, double mt2, double mw2, Conic& q, double& c0,
-                                          double& c1, double& c2) {
-  const double ml2 = fma(l.e, l.e, -fma(l.x, l.x, fma(l.y, l.y, l.z * l.z)));
-  const double mb2 = fma(b.e, b.e, -fma(b.x, b.x, fma(b.y, b.y, b.z * b.z)));
-  const double bl = fma(b.e, l.e, -fma(b.x, l.x, fma(b.y, l.y, b.z * l.z)));
-  const double A = 0.5 * (mw2 - ml2);
-  const double B = fma(0.5, (mt2 - mw2) - mb2, -bl);
-  const double nx = fma(b.e, l.x, -(l.e * b.x)), ny = fma(b.e, l.y, -(l.e * b.y)), nz = fma(b.e, l.z, -(l.e * b.z));
-  const double k = fma(l.e, B, -(b.e * A));
-  const bool ok = fabs(nz) > 1e-12 * b.e * l.e;
-  const double inz = rcp_fast(nz), ile = rcp_fast(l.e);
-  c0 = k * inz; c1 = -nx * inz; c2 = -ny * inz;
-  const double d0 = fma(l.z, c0, A) * ile, d1 = fma(l.z, c1, l.x) * ile, d2 = fma(l.z, c2, l.y) * ile;
-  q.a = fma(d1, d1, -fma(c1, c1, 1.0));
-  q.b = 2.0 * fma(d1, d2, -(c1 * c2));
-  q.c = fma(d2, d2, -fma(c2, c2, 1.0));
-  q.d = 2.0 * fma(d0, d1, -(c0 * c1));
-  q.e = 2.0 * fma(d0, d2, -(c0 * c2));
-  q.f = fma(d0, d0, -(c0 * c0));
-  return ok;
+// ---- variation-independent part of a leg conic ("frame") -------------------------------------------------------------
+// Smearing multiplies the lepton by s_l and the b-jet by s_b.  Then n = E_b l - E_l b scales by s_l s_b, so c1 = -n_x/n_z,
+// c2 = -n_y/n_z, d1, d2 and with them the quadratic part (a, b, c) of the conic do not depend on the variation at all;
+// only c0, d0 and hence (d, e, f) do.  The frame is computed once per event from the nominal four-vectors; per variation
+//   A = (m_W^2 - s_l^2 m_l^2)/2,  B = (m_t^2 - m_W^2 - s_b^2 m_b^2)/2 - s_l s_b (b.l),
+//   c0 = g1 B / s_b - g2 A / s_l  (g1 = E_l / n_z, g2 = E_b / n_z),  d0 = (A / s_l) / E_l + (l_z / E_l) c0.
+struct Frame { double a, b, c, c1, c2, d1, d2, g1, g2, h1, ile, hml2, hmb2, bln; };
+constexpr int FRN = 14;
+__device__ __forceinline__ Frame make_frame(const double* l, const double* b) {   // nominal (px, py, pz, E)
+  Frame F;
+  const double ml2 = fma(l[3], l[3], -fma(l[0], l[0], fma(l[1], l[1], l[2] * l[2])));
+  const double mb2 = fma(b[3], b[3], -fma(b[0], b[0], fma(b[1], b[1], b[2] * b[2])));
+  F.bln = fma(b[3], l[3], -fma(b[0], l[0], fma(b[1], l[1], b[2] * l[2])));
+  const double nx = fma(b[3], l[0], -(l[3] * b[0])), ny = fma(b[3], l[1], -(l[3] * b[1])), nz = fma(b[3], l[2], -(l[3] * b[2]));
+  const bool ok = fabs(nz) > 1e-12 * b[3] * l[3];
+  const double inz = rcp_fast(nz);
+  F.ile = rcp_fast(l[3]);
+  F.c1 = -nx * inz; F.c2 = -ny * inz;
+  F.d1 = fma(l[2], F.c1, l[0]) * F.ile; F.d2 = fma(l[2], F.c2, l[1]) * F.ile;
+  F.a = ok ? fma(F.d1, F.d1, -fma(F.c1, F.c1, 1.0)) : CUDART_NAN;   // NaN conic -> no roots for any pairing using it
+  F.b = 2.0 * fma(F.d1, F.d2, -(F.c1 * F.c2));
+  F.c = fma(F.d2, F.d2, -fma(F.c2, F.c2, 1.0));
+  F.g1 = l[3] * inz; F.g2 = b[3] * inz; F.h1 = l[2] * F.ile;
+  F.hml2 = -0.5 * ml2; F.hmb2 = -0.5 * mb2;
+  return F;
+}
+// (d, e, f) of the conic and c0 of p_z = c0 + c1 p_x + c2 p_y for scales s_l, s_b (rsl = 1/s_l, rsb = 1/s_b);
+// hmw2 = m_W^2 / 2, hcm = (m_t^2 - m_W^2) / 2
+__device__ __forceinline__ void conic_def(const Frame& F, double sl, double sb, double rsl, double rsb, double hmw2, double hcm,
+                                          double& c0, double& d, double& e, double& f) {
+  const double A = fma(F.hml2, sl * sl, hmw2);
+  const double B = fma(-F.bln, sl * sb, fma(F.hmb2, sb * sb, hcm));
+  const double Ar = A * rsl;
+  c0 = fma(F.g1, B * rsb, -(F.g2 * Ar));
+  const double d0 = fma(F.h1, c0, Ar * F.ile);
+  d = 2.0 * fma(d0, F.d1, -(c0 * F.c1));
+  e = 2.0 * fma(d0, F.d2, -(c0 * F.c2));
+  f = fma(d0, d0, -(c0 * c0));
 }
 
 // the conic of leg 2 is in q = MET' - p; rewrite it in p
@@ -393,7 +410,9 @@ __device__ __forceinline__ void best_higgs(const double* ht15, int nb, int i, in
 template <int VC, int NBT>
 struct __align__(16) WarpMem {
   static constexpr int NP = NBT * (NBT - 1) / 2;
-  double con[6][2 * NBT * VC];   // [coefficient][(leg, candidate, variation)]: lanes of a pass differ in the variation
+  double def[3][2 * NBT * VC];   // (d, e, f) of the conic of (leg, candidate, variation); lanes of a pass differ in the variation
+  double fr[FRN][2 * NBT];       // per event: frame of (leg, candidate) incl. the quadratic part (a, b, c)
+  double rs[10 * VC];            // reciprocal scales
   double ht[VC * NP];            // Higgs term of candidate pair (k, l), k < l
   double sc[VC * 10];            // scales of the ten objects
   double M[VC * 2];              // MET'
@@ -409,8 +428,8 @@ __device__ __forceinline__ void score_entry(const WarpMem<VC, NBT>& W, double x,
                                             double& best_ll, uint32_t& best_key) {
   const int vv = tag & 31, i = (tag >> 5) & 7, j = (tag >> 8) & 7, h = (tag >> 11) & 7, t = (tag >> 14) & 15, k = (tag >> 18) & 3;
   const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
-  const Conic A{W.con[0][a1], W.con[1][a1], W.con[2][a1], W.con[3][a1], W.con[4][a1], W.con[5][a1]};
-  const Conic B{W.con[0][a2], W.con[1][a2], W.con[2][a2], W.con[3][a2], W.con[4][a2], W.con[5][a2]};
+  const Conic A{W.fr[0][i], W.fr[1][i], W.fr[2][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
+  const Conic B{W.fr[0][NBT + j], W.fr[1][NBT + j], W.fr[2][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
   double y;
   refine_xy(A, B, x, y);
   const double ll = loglik_of(x, y, W.M[vv], W.M[VC + vv], W.ht[t * VC + vv], inv_lambda);
@@ -434,8 +453,18 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   }
   __syncwarp();
   const int nb = h.n_b, n_pair = nb * (nb - 1) / 2, n_ord = nb * (nb - 1);
+  if (lane < 2 * nb) {               // frames of (leg, candidate): once per event
+    const int leg = lane >= nb, c = lane - leg * nb;
+    const int ls = leg ? 1 - h.lp_slot : h.lp_slot, js = 2 + ((h.cand >> (4 * c)) & 15);
+    const Frame F = make_frame(&W.obj[ls * 4], &W.obj[js * 4]);
+    const int fi = leg * NBT + c;
+    W.fr[0][fi] = F.a; W.fr[1][fi] = F.b; W.fr[2][fi] = F.c; W.fr[3][fi] = F.c1; W.fr[4][fi] = F.c2;
+    W.fr[5][fi] = F.d1; W.fr[6][fi] = F.d2; W.fr[7][fi] = F.g1; W.fr[8][fi] = F.g2; W.fr[9][fi] = F.h1;
+    W.fr[10][fi] = F.ile; W.fr[11][fi] = F.hml2; W.fr[12][fi] = F.hmb2; W.fr[13][fi] = F.bln;
+  }
+  __syncwarp();
   const uint64_t PK = pair_k_list(nb), PL = pair_l_list(nb);
-  const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
+  const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2), inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
   const unsigned lt = (1u << lane) - 1u;
   double best_ll = -CUDART_INF;
   uint32_t best_key = 0xffffffffu;
@@ -452,8 +481,9 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         uint32_t x[4];
         philox4x32_10((uint32_t)h.gidx, (uint32_t)(h.gidx >> 32), (uint32_t)(v0 + vv), 0x54544800u + blk, k0, k1, x);
         double ze, zo; block_normals(x, ze, zo);
-        W.sc[(2 * blk) * VC + vv] = scale_of(W.ks[2 * blk], ze, P.s_min);
-        W.sc[(2 * blk + 1) * VC + vv] = scale_of(W.ks[2 * blk + 1], zo, P.s_min);
+        const double s0 = scale_of(W.ks[2 * blk], ze, P.s_min), s1 = scale_of(W.ks[2 * blk + 1], zo, P.s_min);
+        W.sc[(2 * blk) * VC + vv] = s0; W.sc[(2 * blk + 1) * VC + vv] = s1;
+        W.rs[(2 * blk) * VC + vv] = rcp_fast(s0); W.rs[(2 * blk + 1) * VC + vv] = rcp_fast(s1);
       }
     }
     __syncwarp();
@@ -475,13 +505,17 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       if (vok && comb < 2 * nb) {
         const int leg = comb >= nb, c = comb - leg * nb;
         const int ls = leg ? 1 - h.lp_slot : h.lp_slot, js = 2 + ((h.cand >> (4 * c)) & 15);
-        const V4 l = scale_v4(&W.obj[ls * 4], W.sc[ls * VC + vv]), b = scale_v4(&W.obj[js * 4], W.sc[js * VC + vv]);
-        Conic q; double c0_, c1_, c2_;
-        const bool ok = leg_conic(l, b, mt2, mw2, q, c0_, c1_, c2_);
+        const int fi = leg * NBT + c;
+        Frame F;
+        F.a = W.fr[0][fi]; F.b = W.fr[1][fi]; F.c = W.fr[2][fi]; F.c1 = W.fr[3][fi]; F.c2 = W.fr[4][fi];
+        F.d1 = W.fr[5][fi]; F.d2 = W.fr[6][fi]; F.g1 = W.fr[7][fi]; F.g2 = W.fr[8][fi]; F.h1 = W.fr[9][fi];
+        F.ile = W.fr[10][fi]; F.hml2 = W.fr[11][fi]; F.hmb2 = W.fr[12][fi]; F.bln = W.fr[13][fi];
+        Conic q; double c0_;
+        q.a = F.a; q.b = F.b; q.c = F.c;
+        conic_def(F, W.sc[ls * VC + vv], W.sc[js * VC + vv], W.rs[ls * VC + vv], W.rs[js * VC + vv], hmw2, hcm, c0_, q.d, q.e, q.f);
         if (leg) q = shift_conic(q, W.M[vv], W.M[VC + vv]);
         const int at = (leg * NBT + c) * VC + vv;
-        W.con[0][at] = ok ? q.a : CUDART_NAN;          // NaN conic -> no roots for any pairing that uses it
-        W.con[1][at] = q.b; W.con[2][at] = q.c; W.con[3][at] = q.d; W.con[4][at] = q.e; W.con[5][at] = q.f;
+        W.def[0][at] = q.d; W.def[1][at] = q.e; W.def[2][at] = q.f;
       }
     }
     // ---- H: Higgs term of every unordered candidate pair ---------------------------------------------------------------
@@ -504,8 +538,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       if (vok && ap < n_ord) {
         const int i = ap / (nb - 1); int j = ap - i * (nb - 1); j += (j >= i);
         const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
-        const Conic A{W.con[0][a1], W.con[1][a1], W.con[2][a1], W.con[3][a1], W.con[4][a1], W.con[5][a1]};
-        const Conic B{W.con[0][a2], W.con[1][a2], W.con[2][a2], W.con[3][a2], W.con[4][a2], W.con[5][a2]};
+        const Conic A{W.fr[0][i], W.fr[1][i], W.fr[2][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
+        const Conic B{W.fr[0][NBT + j], W.fr[1][NBT + j], W.fr[2][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
         double g3, g2, g1, g0;
         resultant(A, B, g3, g2, g1, g0);
         mask = solve_quartic(g3, g2, g1, g0, xa, xb);
@@ -629,9 +663,14 @@ reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_id
   const int si = (h.cand >> (4 * i)) & 15, sj = (h.cand >> (4 * j)) & 15;
   const V4 lp = scale_v4(obj[lps], sc[lps]), lm = scale_v4(obj[lms], sc[lms]);
   const V4 bi = scale_v4(obj[2 + si], sc[2 + si]), bj = scale_v4(obj[2 + sj], sc[2 + sj]);
-  Conic A, q2; double c0, c1, c2, e0, e1, e2;
-  leg_conic(lp, bi, mt2, mw2, A, c0, c1, c2);
-  leg_conic(lm, bj, mt2, mw2, q2, e0, e1, e2);
+  // same frame-based construction as the search kernel (identical bits)
+  const double hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2);
+  const Frame F1 = make_frame(obj[lps], obj[2 + si]), F2 = make_frame(obj[lms], obj[2 + sj]);
+  Conic A, q2; double c0, e0;
+  A.a = F1.a; A.b = F1.b; A.c = F1.c; q2.a = F2.a; q2.b = F2.b; q2.c = F2.c;
+  conic_def(F1, sc[lps], sc[2 + si], rcp_fast(sc[lps]), rcp_fast(sc[2 + si]), hmw2, hcm, c0, A.d, A.e, A.f);
+  conic_def(F2, sc[lms], sc[2 + sj], rcp_fast(sc[lms]), rcp_fast(sc[2 + sj]), hmw2, hcm, e0, q2.d, q2.e, q2.f);
+  const double c1 = F1.c1, c2 = F1.c2, e1 = F2.c1, e2 = F2.c2;
   const Conic B = shift_conic(q2, Mx, My);
   double g3, g2, g1, g0, xa[2] = {0, 0}, xb[2] = {0, 0};
   resultant(A, B, g3, g2, g1, g0);
