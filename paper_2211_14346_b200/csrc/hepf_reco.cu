@@ -390,6 +390,11 @@ __device__ __forceinline__ uint32_t make_key(int v, int i, int j, int h, int k) 
 template <int NBT, int VC>
 __device__ __forceinline__ void best_higgs(const double* ht15, int nb, int i, int j, double& ht, int& h, int& kk, int& ll) {
   uint32_t rem = ((1u << nb) - 1u) & ~(1u << i) & ~(1u << j);
+  if (NBT == 4) {                    // exactly one pair is left
+    kk = __ffs(rem) - 1; ll = 31 - __clz(rem); h = 0;
+    ht = ht15[pair_index<NBT>(kk, ll) * VC];
+    return;
+  }
   int r[4], nr = 0;
 #pragma unroll
   for (int c = 0; c < 4; c++) { r[c] = __ffs(rem) - 1; nr += rem != 0; rem &= rem - 1; }
@@ -464,6 +469,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   }
   __syncwarp();
   const uint64_t PK = pair_k_list(nb), PL = pair_l_list(nb);
+  // ap / (nb - 1) for ap < nb (nb - 1) as a multiply-shift: /3 -> *11 >> 5 (ap < 12), /4 -> >> 2, /5 -> *13 >> 6 (ap < 30)
+  const int dmul = nb == 4 ? 11 : (nb == 5 ? 1 : 13), dsh = nb == 4 ? 5 : (nb == 5 ? 2 : 6);
   const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2), inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
   const unsigned lt = (1u << lane) - 1u;
   double best_ll = -CUDART_INF;
@@ -536,7 +543,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       int mask = 0; uint32_t tag = 0;
       double xa[2], xb[2];
       if (vok && ap < n_ord) {
-        const int i = ap / (nb - 1); int j = ap - i * (nb - 1); j += (j >= i);
+        const int i = (ap * dmul) >> dsh; int j = ap - i * (nb - 1); j += (j >= i);   // i = ap / (nb - 1)
         const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
         const Conic A{W.fr[0][i], W.fr[1][i], W.fr[2][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
         const Conic B{W.fr[0][NBT + j], W.fr[1][NBT + j], W.fr[2][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
@@ -798,6 +805,8 @@ extern "C" int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t*
   if (n_variations <= 8 || cfg == 8) rc = launch_search_both<8, 2, 12, 10>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   else if (cfg == 161) rc = launch_search_both<16, 1, 20, 14>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   else if (cfg == 163) rc = launch_search_both<16, 2, 8, 6>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  else if (cfg == 165) rc = launch_search_both<16, 2, 11, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  else if (cfg == 166) rc = launch_search_both<16, 1, 22, 14>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   else if (cfg == 164) rc = launch_search_both<16, 4, 5, 3>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   else rc = launch_search_both<16, 2, 10, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   if (rc != HEPF_OK) return rc;
