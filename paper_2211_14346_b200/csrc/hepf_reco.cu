@@ -58,7 +58,7 @@ template <int NBT> __device__ __forceinline__ int pair_index(int k, int l) { ret
 
 // ---- branch-free FP64 reciprocal / square root / logarithm for the tolerance-compared part of the path ------------
 // MUFU seed (2^-20, measured on B200) + one cubic (rcp) or two quadratic (sqrt) correction steps: <= 1 ulp (rcp) and
-// correctly rounded in every sampled case (sqrt), with 4 resp. 7 FP64-pipe instructions and no slow-path branch.  The
+// correctly rounded in every sampled case (sqrt; argument >= 0 or NaN), with 4 resp. 8 FP64-pipe instructions and no branch.  The
 // smearing (normals, scales, MET') does NOT use these: it keeps the IEEE operations the definition prescribes.
 __device__ __forceinline__ double rcp_fast(double b) {
   double r; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
@@ -66,12 +66,11 @@ __device__ __forceinline__ double rcp_fast(double b) {
   return fma(r, fma(e, e, e), r);
 }
 __device__ __forceinline__ double sqrt_fast(double a) {
-  double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+  double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(fmax(a, 1e-300)));   // a = 0 -> s = 0 exactly, no select
   double h = 0.5 * y, s = a * y;
   const double e = fma(-s, h, 0.5);
   s = fma(s, e, s); h = fma(h, e, h);
-  s = fma(fma(-s, s, a), h, s);
-  return a == 0.0 ? 0.0 : s;
+  return fma(fma(-s, s, a), h, s);
 }
 // ln(a), a > 0 normal: a = m 2^e with m in (sqrt(1/2), sqrt(2)], ln m = 2 atanh(s), s = (m-1)/(m+1); error < 3e-16 relative
 __device__ __forceinline__ double ln_fast(double a) {
@@ -80,9 +79,9 @@ __device__ __forceinline__ double ln_fast(double a) {
   double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(a));
   if (m > 0x1.6a09e667f3bcdp+0) { m *= 0.5; e += 1; }
   const double f = m - 1.0, s = f * rcp_fast(2.0 + f), z = s * s;
-  double p = 2.0 / 19.0;
-  p = fma(p, z, 2.0 / 17.0); p = fma(p, z, 2.0 / 15.0); p = fma(p, z, 2.0 / 13.0); p = fma(p, z, 2.0 / 11.0);
-  p = fma(p, z, 2.0 / 9.0); p = fma(p, z, 2.0 / 7.0); p = fma(p, z, 2.0 / 5.0); p = fma(p, z, 2.0 / 3.0);
+  double p = kLogC[0];
+#pragma unroll
+  for (int k = 1; k < 9; k++) p = fma(p, z, kLogC[k]);
   const double lm = fma(s, p * z, 2.0 * s), ed = (double)e;
   const double r = fma(ed, 0x1.62e42fee00000p-1, fma(ed, 0x1.a39ef35793c76p-33, lm));
   return a > 0.0 ? r : (a == 0.0 ? -CUDART_INF : CUDART_NAN);
@@ -291,6 +290,7 @@ __device__ __noinline__ double root_y_fallback(const Conic k1, const Conic k2, d
 
 // one Newton step on the pair of conics in (x, y); mv = |dx| + |dy| (left unchanged, and the point kept, if the
 // Jacobian is singular)
+template <bool GUARD>
 __device__ __forceinline__ void newton_xy(const Conic& A, const Conic& B, double& x, double& y, double& mv) {
   const double t1 = fma(A.a, x, fma(A.b, y, A.d)), t2 = fma(A.c, y, A.e);
   const double F1 = fma(t1, x, fma(t2, y, A.f)), F1x = fma(A.a, x, t1), F1y = fma(A.b, x, fma(A.c, y, t2));
@@ -299,14 +299,18 @@ __device__ __forceinline__ void newton_xy(const Conic& A, const Conic& B, double
   const double idet = rcp_fast(fma(F1x, F2y, -(F1y * F2x)));
   const double dx = fma(F1, F2y, -(F2 * F1y)) * idet, dy = fma(F1x, F2, -(F2x * F1)) * idet;
   const double m = fabs(dx) + fabs(dy);
-  const bool fin = m <= CUDART_MAX_NORMAL_F;
-  x = fin ? x - dx : x; y = fin ? y - dy : y; mv = fin ? m : 0.0;
+  if (GUARD) {
+    const bool fin = m <= CUDART_MAX_NORMAL_F;
+    x = fin ? x - dx : x; y = fin ? y - dy : y; mv = fin ? m : 0.0;
+  } else {                           // hot path: a singular Jacobian turns the point into NaN, which never wins the argmax
+    x -= dx; y -= dy; mv = m;
+  }
 }
 __device__ __noinline__ double2 refine_more(const Conic A, const Conic B, double x, double y) {
 #pragma unroll 1
   for (int it = 0; it < 6; it++) {
     double mv = 0.0;
-    newton_xy(A, B, x, y, mv);
+    newton_xy<true>(A, B, x, y, mv);
     if (mv <= 1e-10 * (fabs(x) + fabs(y))) break;
   }
   return make_double2(x, y);
@@ -322,7 +326,7 @@ __device__ __forceinline__ void refine_xy(const Conic& A, const Conic& B, double
   else y = root_y_fallback(A, B, x);
   double mv = 0.0;
 #pragma unroll
-  for (int it = 0; it < 2; it++) newton_xy(A, B, x, y, mv);
+  for (int it = 0; it < 2; it++) newton_xy<false>(A, B, x, y, mv);
   // a second step that still moved the point by more than 1e-10 (relative) means near-tangent conics (linear
   // convergence): keep polishing out of line, up to six more steps
   if (mv > 1e-10 * (fabs(x) + fabs(y))) { const double2 r = refine_more(A, B, x, y); x = r.x; y = r.y; }
