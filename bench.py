@@ -32,11 +32,55 @@ UNIT = "reconstructions/s"
 FP64_LANES_PER_SM = 64
 # Algorithmic FP64 work of one solve: the search kernel's own predicated-on thread-level FP64 instruction counts per
 # solve (idle lanes and divergence waste do not count), from the committed ncu capture of this build
-# (profiles/r01c_reco_search.md): DADD + DMUL + DFMA lane-ops, and flop with FMA = 2.  DESIGN.md section 7.
-FP64_OPS_PER_SOLVE = {"dadd": 36.1, "dmul": 93.7, "dfma": 171.5}
-LANE_OPS_PER_SOLVE = sum(FP64_OPS_PER_SOLVE.values())
-FLOP_PER_SOLVE = FP64_OPS_PER_SOLVE["dadd"] + FP64_OPS_PER_SOLVE["dmul"] + 2.0 * FP64_OPS_PER_SOLVE["dfma"]
-DRAM_BYTES_PER_LAUNCH = 274.6e6   # ncu dram__bytes_read.sum + dram__bytes_write.sum of the search kernel (same profile)
+# (profiles/r01d_reco_search.md): DADD + DMUL + DFMA lane-ops, and flop with FMA = 2.  DESIGN.md section 7.
+FP64_OPS_PER_SOLVE = {"dadd": 32.6, "dmul": 81.9, "dfma": 158.2}
+FP64_OPS_PER_SOLVE_NB6 = {"dadd": 26.4, "dmul": 68.1, "dfma": 129.6}   # n_b = 6 kernel (cfg3), profiles/r01d
+DRAM_BYTES_PER_LAUNCH = 276.2e6   # ncu dram__bytes_read.sum + dram__bytes_write.sum of the search kernel (same profile)
+
+
+def chain_bytes_per_event(chain) -> int:
+    """Algorithmic bytes hepf_select must read per event: flags + the columns the chain names."""
+    need = set()
+    for kind, *_ in chain:
+        if kind == hs.LEP_PT_GT: need.add("lep_pt")
+        elif kind == hs.LEP_ABSETA_LT: need.add("lep_eta")
+        elif kind in (hs.NJET_GE, hs.NBJET_GE): need.update(("jet_pt", "jet_eta"))
+        elif kind == hs.MET_GT: need.add("met")
+        elif kind in (hs.MLL_GT, hs.MLL_OUTSIDE): need.add("mll")
+    size = {"lep_pt": 16, "lep_eta": 16, "jet_pt": 64, "jet_eta": 64, "met": 8, "mll": 8}
+    return 4 + sum(size[c] for c in need)
+
+
+def run_philox(args):
+    """--workload cfg5: standalone hepf_philox_normal stream (BASELINE.json configs[4]), normals/s and GB/s written."""
+    import torch
+    import paper_2211_14346_b200 as hepf
+    hepf.load()
+    torch.cuda.set_device(0)
+    n = args.events or hs.PHILOX_CFG5["n"]
+    out = torch.empty(n, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    for _ in range(max(3, args.warmup)):
+        hepf.philox_normal(hs.PHILOX_CFG5["seed"], 0, n, out=out, stream=stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        hepf.philox_normal(hs.PHILOX_CFG5["seed"], 0, n, out=out, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    gbs = 8.0 * n / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "standard-normal FP64 draws/sec (Philox4x32-10 + Box-Muller)", "value": n / (ms * 1e-3),
+                      "unit": "normals/s", "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": f"cfg5: {n} normals, seed 7, counter 0", "l2": "34 GB written per step, far larger than L2"},
+                      "gpu_launches": args.steps,
+                      "roofline": {"bound": "hbm", "kernel": "philox_normal_kernel<true>", "achieved": gbs, "peak": hbm,
+                                   "unit": "GB/s", "frac": gbs / hbm, "traffic": None,
+                                   "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy, read+write)" if peaks else "fallback 6650"}}))
 
 
 def solves_of(store, idx, n_variations: int) -> int:
@@ -91,7 +135,7 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def cpu_oracle_rate(store, idx, n_variations, seed, target_s=15.0):
+def cpu_oracle_rate(store, idx, n_variations, seed, target_s=15.0, chain=hs.CHAIN_BASE):
     """Time the oracle, as it stands, on a bounded sample of the same workload on the host cores."""
     import oracle
     cores = os.cpu_count() or 1
@@ -101,7 +145,7 @@ def cpu_oracle_rate(store, idx, n_variations, seed, target_s=15.0):
     m = int(min(len(idx), max(2048, 2048 * target_s / dt)))
     sample = idx[:m]
     t0 = time.perf_counter()
-    oracle.select(store, hs.CHAIN_BASE)            # the oracle's selection of the whole batch is part of a step
+    oracle.select(store, chain)                    # the oracle's selection of the whole batch is part of a step
     t_sel = time.perf_counter() - t0
     t0 = time.perf_counter(); oracle.reconstruct_tth(store, sample, n_variations, seed, n_threads=cores)
     dt = time.perf_counter() - t0
@@ -148,10 +192,12 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="hepf", choices=["hepf", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.workload == "cfg5":
+        return run_philox(args)
     cfg = hs.CONFIGS[int(args.workload[3])]
     if args.impl == "reference":
         return run_reference(args, cfg, args.workload)
@@ -211,12 +257,12 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     mids = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     binding.timing_enable(True)
-    k_search, k_final, k_sel = [], [], []
+    k_search, k_search6, k_final, k_sel, k_sel_eval = [], [], [], [], []
     e0.record(stream)
     for s in range(args.steps):
         step(mids[s])
         # device time of each kernel of this step, from events the library records on the stream around its launches
-        k_search.append(binding.timing_ms(3, 4)); k_final.append(binding.timing_ms(5, 6)); k_sel.append(binding.timing_ms(0, 2))
+        k_search.append(binding.timing_ms(3, 4)); k_search6.append(binding.timing_ms(4, 5)); k_final.append(binding.timing_ms(5, 6)); k_sel.append(binding.timing_ms(0, 2)); k_sel_eval.append(binding.timing_ms(0, 1))
     e1.record(stream)
     torch.cuda.synchronize()
     binding.timing_enable(False)
@@ -273,31 +319,42 @@ def main():
     p0.record(stream); binding.fp64_peak_probe(sms * 8, 256, per_thread, sink, stream); p1.record(stream)
     torch.cuda.synchronize()
     fma_peak = 2.0 * sms * 8 * 256 * per_thread / (p0.elapsed_time(p1) * 1e-3) / 1e12
-    ms_search = float(np.mean(k_search))
+    nb6 = float(np.mean(k_search6)) > float(np.mean(k_search))     # which candidate-count class dominates this workload
+    ms_search = float(np.mean(k_search6 if nb6 else k_search))
+    ops = FP64_OPS_PER_SOLVE_NB6 if nb6 else FP64_OPS_PER_SOLVE
+    LANE_OPS_PER_SOLVE = sum(ops.values()); FLOP_PER_SOLVE = ops["dadd"] + ops["dmul"] + 2.0 * ops["dfma"]
     achieved = FLOP_PER_SOLVE * n_solves / (ms_search * 1e-3) / 1e12
     lane_rate = LANE_OPS_PER_SOLVE * n_solves / (ms_search * 1e-3)
     lane_peak = sms * FP64_LANES_PER_SM * sm_max * 1e6
-    roofline = {"bound": "alu", "kernel": "reco_search_kernel<16,4>", "achieved": achieved, "peak": peak_tflops,
-                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": DRAM_BYTES_PER_LAUNCH,
+    roofline = {"bound": "alu", "kernel": "reco_search_kernel<16,6>" if nb6 else "reco_search_kernel<16,4>", "achieved": achieved, "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": DRAM_BYTES_PER_LAUNCH if args.workload == "cfg2" else None,
                 "peak_source": f"{sms} SMs x {FP64_LANES_PER_SM} FP64 FMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md section 6.2)",
                 "dfma_chain_measured_tflops": fma_peak, "frac_of_measured_dfma": achieved / fma_peak,
                 "fp64_lane_ops_per_solve": LANE_OPS_PER_SOLVE, "flop_per_solve": FLOP_PER_SOLVE,
                 "fp64_pipe_frac": lane_rate / lane_peak, "kernel_ms": ms_search,
                 "kernel_share_of_step": ms_search / ms_per_step,
-                "other_kernels_ms": {"select_eval+scatter": float(np.mean(k_sel)), "reco_finalize": float(np.mean(k_final)),
+                "other_kernels_ms": {"reco_search_other_class": float(np.mean(k_search if nb6 else k_search6)), "select_eval+scatter": float(np.mean(k_sel)), "reco_finalize": float(np.mean(k_final)),
                                      "hepf_reconstruct_tth_call": ms_reco}}
+    sel_bytes = chain_bytes_per_event(cfg.cuts) * n + 4 * n_sel
+    sel_ms = float(np.mean(k_sel_eval))
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    hbm_peak = float(json.load(open(peaks_path)).get("hbm_gbs", 6650.0)) if os.path.exists(peaks_path) else 6650.0
+    select_line = {"kernel": "select_eval_kernel", "events_per_s": n / (sel_ms * 1e-3), "bound": "hbm",
+                   "achieved": sel_bytes / (sel_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                   "frac": sel_bytes / (sel_ms * 1e-3) / 1e9 / hbm_peak, "algorithmic_bytes": sel_bytes, "kernel_ms": sel_ms,
+                   "eval+scatter_ms": float(np.mean(k_sel))}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",
            "config": {"workload": f"{args.workload}: {cfg.name}", "events_per_gpu": n, "selected_per_gpu": n_sel,
-                      "n_variations": V, "pairings": 12 if cfg.n_fake_b == 0 else 30, "solves_per_step": all_solves,
+                      "n_variations": V, "pairings": 12 if cfg.n_fake_b == 0 else 30, "variations": V, "solves_per_step": all_solves,
                       "l2": "inputs (516 B/event x 1e6 = 516 MB) larger than the 126 MB L2; no flush needed",
                       "parallelism": f"dp{world} (events sharded by global index, no collective)"},
-           "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
+           "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "select": select_line}
     if not args.no_cpu_baseline and world == 1:
-        out["cpu_baseline"] = cpu_oracle_rate(store, idx_host, V, seed)
+        out["cpu_baseline"] = cpu_oracle_rate(store, idx_host, V, seed, chain=cfg.cuts)
     elif not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_oracle_rate(store, idx_host, V, seed, target_s=8.0)
+        out["cpu_baseline"] = cpu_oracle_rate(store, idx_host, V, seed, target_s=8.0, chain=cfg.cuts)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
