@@ -182,7 +182,8 @@ __device__ __forceinline__ float cos_third_acos(float c) {
   p = fmaf(p, a, 0.0066700901f); p = fmaf(p, a, -0.0170881256f); p = fmaf(p, a, 0.0308918810f);
   p = fmaf(p, a, -0.0501743046f); p = fmaf(p, a, 0.0889789874f); p = fmaf(p, a, -0.2145988016f);
   p = fmaf(p, a, 1.5707963050f);
-  float phi = sqrtf(1.0f - a) * p;
+  const float om = fmaxf(1.0f - a, 1e-30f);
+  float phi = om * rsqrtf(om) * p;
   phi = (c < 0.0f) ? 3.14159265f - phi : phi;
   const float t = phi * (1.0f / 3.0f), z = t * t;
   float q = -1.0f / 3628800.0f;
@@ -202,14 +203,17 @@ __device__ __forceinline__ double resolvent_seed(double p, double q, double r) {
   const float P3 = (c1 - pf * p3) * (1.0f / 3.0f);
   const float u = -0.5f * fmaf(2.0f * p3 * p3, p3, fmaf(-p3, c1, c0));
   const float D = fmaf(u, u, P3 * P3 * P3);
-  float w;
+  float w;                           // MUFU-grade arithmetic is enough for a seed: rsqrt / rcp / lg2 / ex2 approximations
   if (D > 0.0f) {
-    const float A = cbrtf(u + copysignf(sqrtf(D), u));
-    w = (A != 0.0f) ? A - P3 / A : 0.0f;
+    const float t = fabsf(u) + D * rsqrtf(D);
+    float A = exp2f(__log2f(t) * (1.0f / 3.0f));                     // cbrt(t), then one Newton step
+    A = A - __fdividef(fmaf(A * A, A, -t), 3.0f * A * A);
+    A = copysignf(A, u);
+    w = A - __fdividef(P3, A);
   } else {
-    const float rho = sqrtf(-P3);
-    const float ct = fminf(1.0f, fmaxf(-1.0f, u / (rho * rho * rho)));
-    w = (rho > 0.0f) ? 2.0f * rho * cos_third_acos(ct) : 0.0f;
+    const float rr = rsqrtf(fmaxf(-P3, 1e-30f)), rho = -P3 * rr;    // rho = sqrt(-P3), rr = 1 / rho
+    const float ct = fminf(1.0f, fmaxf(-1.0f, u * rr * rr * rr));
+    w = 2.0f * rho * cos_third_acos(ct);
   }
   return (double)(w - p3) * pow2(2 * E);
 }
@@ -228,6 +232,19 @@ __device__ __noinline__ double resolvent_root_from_above(double p, double tp, do
     if (step <= 1e-15 * m) break;
   }
   return m;
+}
+
+// The FP32-seeded iterate has not converged onto a positive root yet: a few more Newton steps from where it stands
+// (the usual case: the seed lost digits to cancellation), and only then the monotone route from above.
+__device__ __noinline__ double resolvent_rescue(double m, double p, double tp, double c1, double c0) {
+#pragma unroll 1
+  for (int it = 0; it < 5; it++) {
+    const double f = fma(fma(m + p, m, c1), m, c0), df = fma(fma(3.0, m, tp), m, c1);
+    const double step = f * rcp_fast(df);
+    m -= step;
+    if (fabs(step) <= 1e-8 * m) return m;
+  }
+  return resolvent_root_from_above(p, tp, c1, c0);
 }
 
 struct Biquad { double x[4]; int mask; };
@@ -259,7 +276,7 @@ __device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, do
   }
   // The seed is only FP32: accept the iterate if the last step was a converged one onto a positive root (any positive
   // root of the resolvent gives a real factorisation); otherwise take the slow, monotone route (rare).
-  if (!(fabs(step) <= 1e-8 * m)) m = resolvent_root_from_above(p, tp, c1, c0);
+  if (!(fabs(step) <= 1e-8 * m)) m = resolvent_rescue(m, p, tp, c1, c0);
   int mask = 0;
   if (m > 0.0) {
     const double s = sqrt_fast(2.0 * m), qs = q * rcp_fast(s);          // 2 qs' with qs' = q / (2 s)
