@@ -269,7 +269,7 @@ __device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, do
   const double c1 = fma(0.25 * p, p, -r), c0 = -0.125 * q * q, tp = 2.0 * p;
   double m = resolvent_seed(p, q, r), step = 0.0;
 #pragma unroll
-  for (int it = 0; it < 3; it++) {   // FP64 Newton on the resolvent cubic
+  for (int it = 0; it < 2; it++) {   // FP64 Newton on the resolvent cubic
     const double f = fma(fma(m + p, m, c1), m, c0), df = fma(fma(3.0, m, tp), m, c1);
     step = f * rcp_fast(df);
     m -= step;
