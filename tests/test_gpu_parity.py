@@ -263,3 +263,57 @@ def test_cfg2_full_size_sampled_parity(hepf):
     sample = np.arange(0, n, 400)
     want, aux = oracle.reconstruct_tth(st, idx[sample], cfg.n_variations, cfg.reco_seed, n_threads=8)
     assert_parity(st, got[sample], want, aux, cfg.n_variations, cfg.reco_seed, label="cfg2-sampled")
+
+
+def test_cfg3_full_size_sampled_parity(hepf):
+    """BASELINE.json configs[2] (10^6 events, 6 b candidates, V = 256) in the launch configuration bench.py times:
+    selection exact for all events, a 1-in-4000 sample of the records against the oracle, closure on quantiles."""
+    cfg = hs.CONFIGS[3]
+    st = cfg.events()
+    want_idx, want_cf = oracle.select(st, cfg.cuts)
+    dev, idx_t, n, idx, cf = _gpu_select(hepf, st, cfg.cuts)
+    assert np.array_equal(idx, want_idx) and np.array_equal(cf, want_cf)
+    got = _gpu_reco(hepf, dev, idx_t, n, cfg.n_variations, cfg.reco_seed)
+    assert np.array_equal(got["event"], idx)
+    solved = (got["status"] & 1) == 1
+    assert solved.mean() > 0.95
+    for f, m in (("m_top", 172.5), ("m_antitop", 172.5), ("m_wplus", 80.4), ("m_wminus", 80.4)):
+        err = np.abs(got[f][solved] - m) / m
+        assert np.median(err) < 1e-13 and np.quantile(err, 0.99) < 1e-9
+    sample = np.arange(0, n, 4000)
+    want, aux = oracle.reconstruct_tth(st, idx[sample], cfg.n_variations, cfg.reco_seed, n_threads=16)
+    assert_parity(st, got[sample], want, aux, cfg.n_variations, cfg.reco_seed, max_excused_frac=0.03, label="cfg3-sampled")
+
+
+def test_cfg4_full_size_select_exact_and_survivor_parity(hepf):
+    """BASELINE.json configs[3]: 2*10^7 events, 30 % background, the tightened 8-cut chain (~5 % pass).  Survivor
+    indices and cutflow are compared exactly for ALL events; the reconstruction of a 1-in-1000 sample of the survivors
+    (V = 16) against the oracle."""
+    cfg = hs.CONFIGS[4]
+    st = cfg.events()
+    want_idx, want_cf = oracle.select(st, cfg.cuts)
+    dev, idx_t, n, idx, cf = _gpu_select(hepf, st, cfg.cuts)
+    assert n == len(want_idx) and 0.03 < n / st.n_events < 0.07
+    assert np.array_equal(idx, want_idx) and np.array_equal(cf, want_cf)
+    assert all(a >= b for a, b in zip(cf, cf[1:])) and cf[-1] == n
+    got = _gpu_reco(hepf, dev, idx_t, n, cfg.n_variations, cfg.reco_seed)
+    assert np.array_equal(got["event"], idx)
+    sample = np.arange(0, n, 1000)
+    want, aux = oracle.reconstruct_tth(st, idx[sample], cfg.n_variations, cfg.reco_seed, n_threads=16)
+    assert_parity(st, got[sample], want, aux, cfg.n_variations, cfg.reco_seed, max_excused_frac=0.01, label="cfg4-sampled")
+
+
+def test_cfg5_full_stream_sampled_windows(hepf):
+    """BASELINE.json configs[4]: all 2^32 normals of the (seed 7, counter 0) stream in one call; the 2^20 prefix and
+    windows near 2^31, 2^32 - 4096 and at odd offsets are compared bit for bit with the oracle."""
+    import torch
+    n = hs.PHILOX_CFG5["n"]
+    free, _ = torch.cuda.mem_get_info()
+    if free < 8 * n + (1 << 30):
+        pytest.skip("not enough device memory for 2^32 doubles")
+    out = hepf.philox_normal(7, 0, n)
+    torch.cuda.synchronize()
+    for start, m in ((0, 1 << 20), ((1 << 31) - 2048, 4096), (n - 4096, 4096), (123_456_789, 4097), (3_000_000_001, 1000)):
+        got = out[start:start + m].cpu().numpy()
+        assert got.tobytes() == oracle.philox_normal(7, start, m).tobytes(), start
+    del out
