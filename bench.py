@@ -165,7 +165,7 @@ def run_reference(args, cfg, name):
     n_ev = min(cfg.n_events, 200_000)
     store = cfg.events(n_ev)
     idx, _ = oracle.select(store, cfg.cuts)
-    per_step = max(16, int(len(idx) * 0.0 + 400))
+    per_step = min(4000, max(16, len(idx) // 2))
     times, solves = [], 0
     for s in range(args.warmup + args.steps):
         sample = idx[(s * per_step) % max(1, len(idx) - per_step):][:per_step]
@@ -180,7 +180,7 @@ def run_reference(args, cfg, name):
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
                       "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / max(1, args.steps),
                       "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                      "config": {"workload": name, "n_variations": cfg.n_variations, "sample": sample_txt},
+                      "config": {"workload": cfg.name, "n_variations": cfg.n_variations, "sample": sample_txt},
                       "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample_txt},
                       "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
                       "gpu_launches": 0}))
@@ -346,7 +346,7 @@ def main():
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",
-           "config": {"workload": f"{args.workload}: {cfg.name}", "events_per_gpu": n, "selected_per_gpu": n_sel,
+           "config": {"workload": cfg.name, "events_per_gpu": n, "selected_per_gpu": n_sel,
                       "n_variations": V, "pairings": 12 if cfg.n_fake_b == 0 else 30, "variations": V, "solves_per_step": all_solves,
                       "l2": "inputs (516 B/event x 1e6 = 516 MB) larger than the 126 MB L2; no flush needed",
                       "parallelism": f"dp{world} (events sharded by global index, no collective)"},
