@@ -195,6 +195,8 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variations", type=int, default=0, help="override the workload's V (SURVEY 8(f) NEXT-1: 128 = ttH_scinp, 1024 = ttH_sci)")
+    ap.add_argument("--sigma-scale", type=float, default=None, help="0 = no smearing, the paper's ttH_as variant")
     args = ap.parse_args()
     if args.workload == "cfg5":
         return run_philox(args)
@@ -220,7 +222,8 @@ def main():
     # weak scaling: rank r owns global events [r n, (r+1) n); the Philox keys use the global index
     store = cfg.events(n_ev, first_event=rank * n_ev)
     dev = hepf.DeviceEvents.from_host(store)
-    n, V, seed = store.n_events, cfg.n_variations, cfg.reco_seed
+    n, V, seed = store.n_events, (args.variations or cfg.n_variations), cfg.reco_seed
+    params = hepf.default_params(sigma_scale=args.sigma_scale) if args.sigma_scale is not None else None
     stream = torch.cuda.current_stream()
     out_idx = torch.empty(max(n, 1), dtype=torch.int32, device="cuda")
     out_count = torch.zeros(1, dtype=torch.int64, device="cuda")
@@ -237,7 +240,7 @@ def main():
         n_sel = int(count_host[0])
         if ev_mid is not None:
             ev_mid[0].record(stream)
-        hepf.reconstruct_tth(dev, out_idx, n_sel, V, seed, out_best=out_best, ws=reco_ws, stream=stream)
+        hepf.reconstruct_tth(dev, out_idx, n_sel, V, seed, params, out_best=out_best, ws=reco_ws, stream=stream)
         if ev_mid is not None:
             ev_mid[1].record(stream)
         return n_sel
@@ -287,14 +290,14 @@ def main():
     arena = torch.empty(binding.tth_host_arena_bytes(n, V) + 512, dtype=torch.uint8, device="cuda")
     hb = torch.empty((max(n, 1), 128), dtype=torch.uint8).pin_memory()
     hi = torch.empty(max(n, 1), dtype=torch.int32).pin_memory()
-    hepf.tth_host(hstore, cfg.cuts, V, seed, arena=arena, out_best=hb, out_idx=hi, stream=stream)
+    hepf.tth_host(hstore, cfg.cuts, V, seed, params, arena=arena, out_best=hb, out_idx=hi, stream=stream)
     e2e_steps = max(1, min(args.steps, 3))
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        hepf.tth_host(hstore, cfg.cuts, V, seed, arena=arena, out_best=hb, out_idx=hi, stream=stream)
+        hepf.tth_host(hstore, cfg.cuts, V, seed, params, arena=arena, out_best=hb, out_idx=hi, stream=stream)
     torch.cuda.synchronize()
     te = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device="cuda")
     if world > 1:
