@@ -154,21 +154,30 @@ __device__ __forceinline__ Lines lines_of(const Conic& k1, const Conic& k2) {
   return L;
 }
 
+// The part of the resultant that only depends on the quadratic coefficients of the two conics, i.e. (frames) on the
+// event and the pairing but not on the variation: p2, q1, r3 and 1 / h4.  Computed once per event and pairing; it also
+// takes the reciprocal off the critical path of stage C.
+struct PairConst { double p2, q1, r3, ih4; };
+__device__ __forceinline__ PairConst pair_consts(double a1, double b1, double c1, double a2, double b2, double c2) {
+  PairConst K;
+  K.p2 = fma(c1, a2, -(c2 * a1)); K.q1 = fma(c1, b2, -(c2 * b1)); K.r3 = fma(b1, a2, -(b2 * a1));
+  K.ih4 = rcp_fast(fma(K.p2, K.p2, -(K.q1 * K.r3)));   // h4 == 0 -> NaN coefficients -> no roots
+  return K;
+}
 // resultant of the two conics in x (y eliminated) as a MONIC quartic x^4 + g3 x^3 + g2 x^2 + g1 x + g0
-__device__ __forceinline__ void resultant(const Conic& k1, const Conic& k2, double& g3, double& g2, double& g1, double& g0) {
-  const Lines L = lines_of(k1, k2);
+__device__ __forceinline__ void resultant(const Conic& k1, const Conic& k2, const PairConst& K, double& g3, double& g2,
+                                          double& g1, double& g0) {
+  const double p0 = fma(k1.c, k2.f, -(k2.c * k1.f)), p1 = fma(k1.c, k2.d, -(k2.c * k1.d));
+  const double q0 = fma(k1.c, k2.e, -(k2.c * k1.e));
   const double r0 = fma(k1.e, k2.f, -(k2.e * k1.f));
   const double r1 = fma(k1.e, k2.d, fma(k1.b, k2.f, -fma(k2.e, k1.d, k2.b * k1.f)));
   const double r2 = fma(k1.e, k2.a, fma(k1.b, k2.d, -fma(k2.e, k1.a, k2.b * k1.d)));
-  const double r3 = fma(k1.b, k2.a, -(k2.b * k1.a));
-  const double tp0 = 2.0 * L.p0, tp1 = 2.0 * L.p1;
-  const double h0 = fma(L.p0, L.p0, -(L.q0 * r0));
-  const double h1 = fma(tp0, L.p1, -fma(L.q0, r1, L.q1 * r0));
-  const double h2 = fma(tp0, L.p2, fma(L.p1, L.p1, -fma(L.q0, r2, L.q1 * r1)));
-  const double h3 = fma(tp1, L.p2, -fma(L.q0, r3, L.q1 * r2));
-  const double h4 = fma(L.p2, L.p2, -(L.q1 * r3));
-  const double ih4 = rcp_fast(h4);   // h4 == 0 -> inf/NaN coefficients -> every discriminant test below is false
-  g0 = h0 * ih4; g1 = h1 * ih4; g2 = h2 * ih4; g3 = h3 * ih4;
+  const double tp0 = 2.0 * p0, tp1 = 2.0 * p1;
+  const double h0 = fma(p0, p0, -(q0 * r0));
+  const double h1 = fma(tp0, p1, -fma(q0, r1, K.q1 * r0));
+  const double h2 = fma(tp0, K.p2, fma(p1, p1, -fma(q0, r2, K.q1 * r1)));
+  const double h3 = fma(tp1, K.p2, -fma(q0, K.r3, K.q1 * r2));
+  g0 = h0 * K.ih4; g1 = h1 * K.ih4; g2 = h2 * K.ih4; g3 = h3 * K.ih4;
 }
 
 __device__ __forceinline__ int exp_of(double v) { return ((__double2hiint(v) >> 20) & 0x7ff) - 1023; }
@@ -439,6 +448,7 @@ struct __align__(16) WarpMem {
   double def[3][2 * NBT * VC];   // (d, e, f) of the conic of (leg, candidate, variation); lanes of a pass differ in the variation
   double fr[FRN][2 * NBT];       // per event: frame of (leg, candidate) incl. the quadratic part (a, b, c)
   double rs[10 * VC];            // reciprocal scales
+  double pc[4][NBT * (NBT - 1)];  // per event: pair constants (p2, q1, r3, 1/h4) of every ordered pairing
   double ht[VC * NP];            // Higgs term of candidate pair (k, l), k < l
   double sc[VC * 10];            // scales of the ten objects
   double M[VC * 2];              // MET'
@@ -492,6 +502,12 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   const uint64_t PK = pair_k_list(nb), PL = pair_l_list(nb);
   // ap / (nb - 1) for ap < nb (nb - 1) as a multiply-shift: /3 -> *11 >> 5 (ap < 12), /4 -> >> 2, /5 -> *13 >> 6 (ap < 30)
   const int dmul = nb == 4 ? 11 : (nb == 5 ? 1 : 13), dsh = nb == 4 ? 5 : (nb == 5 ? 2 : 6);
+  if (lane < n_ord) {                // pair constants of every ordered pairing: once per event
+    const int i = (lane * dmul) >> dsh; int j = lane - i * (nb - 1); j += (j >= i);
+    const PairConst K = pair_consts(W.fr[0][i], W.fr[1][i], W.fr[2][i], W.fr[0][NBT + j], W.fr[1][NBT + j], W.fr[2][NBT + j]);
+    W.pc[0][lane] = K.p2; W.pc[1][lane] = K.q1; W.pc[2][lane] = K.r3; W.pc[3][lane] = K.ih4;
+  }
+  __syncwarp();
   const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2), inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
   const unsigned lt = (1u << lane) - 1u;
   double best_ll = -CUDART_INF;
@@ -568,8 +584,9 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
         const Conic A{W.fr[0][i], W.fr[1][i], W.fr[2][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
         const Conic B{W.fr[0][NBT + j], W.fr[1][NBT + j], W.fr[2][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
+        const PairConst K{W.pc[0][ap], W.pc[1][ap], W.pc[2][ap], W.pc[3][ap]};
         double g3, g2, g1, g0;
-        resultant(A, B, g3, g2, g1, g0);
+        resultant(A, B, K, g3, g2, g1, g0);
         mask = solve_quartic(g3, g2, g1, g0, xa, xb);
         if (mask) {
           double ht; int hh, kk, ll;
@@ -701,7 +718,7 @@ reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_id
   const double c1 = F1.c1, c2 = F1.c2, e1 = F2.c1, e2 = F2.c2;
   const Conic B = shift_conic(q2, Mx, My);
   double g3, g2, g1, g0, xa[2] = {0, 0}, xb[2] = {0, 0};
-  resultant(A, B, g3, g2, g1, g0);
+  resultant(A, B, pair_consts(A.a, A.b, A.c, B.a, B.b, B.c), g3, g2, g1, g0);
   const int mask = solve_quartic(g3, g2, g1, g0, xa, xb);
   double xs[4], ys[4]; int nr = 0;
   if (mask & 1) { xs[0] = xa[0]; xs[1] = xa[1]; nr = 2; }
