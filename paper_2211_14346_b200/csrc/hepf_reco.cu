@@ -66,7 +66,8 @@ __device__ __forceinline__ double rcp_fast(double b) {
   return fma(r, fma(e, e, e), r);
 }
 __device__ __forceinline__ double sqrt_fast(double a) {
-  double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(fmax(a, 1e-300)));   // a = 0 -> s = 0 exactly, no select
+  // the seed is taken of a + 1e-300 (== a for every a > 1e-284): a = 0 then gives s = 0 * 1e150 = 0 exactly, no select
+  double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a + 1e-300));
   double h = 0.5 * y, s = a * y;
   const double e = fma(-s, h, 0.5);
   s = fma(s, e, s); h = fma(h, e, h);
