@@ -104,7 +104,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                          "--format=csv,noheader,nounits", "-lms", "50"], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -189,8 +189,8 @@ def run_reference(args, cfg, name):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="hepf", choices=["hepf", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (debugging)")
@@ -291,7 +291,7 @@ def main():
     hb = torch.empty((max(n, 1), 128), dtype=torch.uint8).pin_memory()
     hi = torch.empty(max(n, 1), dtype=torch.int32).pin_memory()
     hepf.tth_host(hstore, cfg.cuts, V, seed, params, arena=arena, out_best=hb, out_idx=hi, stream=stream)
-    e2e_steps = max(1, min(args.steps, 3))
+    e2e_steps = max(1, min(args.steps, 10))
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
@@ -351,7 +351,7 @@ def main():
            "data": "synthetic",
            "config": {"workload": cfg.name, "events_per_gpu": n, "selected_per_gpu": n_sel,
                       "n_variations": V, "pairings": 12 if cfg.n_fake_b == 0 else 30, "variations": V, "solves_per_step": all_solves,
-                      "l2": "inputs (516 B/event x 1e6 = 516 MB) larger than the 126 MB L2; no flush needed",
+                      "l2": (f"inputs ({516 * n / 1e6:.0f} MB of columns) larger than the 126 MB L2; no flush needed" if 516 * n > 126e6 else f"inputs ({516 * n / 1e6:.1f} MB) fit in L2: parity-test configuration, not a bench line"),
                       "parallelism": f"dp{world} (events sharded by global index, no collective)"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "select": select_line}
     if not args.no_cpu_baseline and world == 1:

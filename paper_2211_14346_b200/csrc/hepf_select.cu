@@ -13,7 +13,7 @@
 //   K2 select_scatter: each block sums the counts of the blocks before it (<= 1184 values), then replays its
 //                      range from the 1-bit-per-event masks (1/1440 of K1's traffic) and writes the ascending
 //                      index list with popc-prefix offsets.  Deterministic, no atomics on the index cursor.
-// Each block owns a contiguous range of 512-event tiles; the grid is 8 blocks per SM (one wave).
+// Each block owns a contiguous range of 512-event tiles; the grid is one wave of resident blocks (occupancy query: 2 per SM at 111 registers).
 #include "hepf_common.cuh"
 
 namespace hepf {
@@ -174,9 +174,10 @@ select_scatter_kernel(int64_t n_tiles, int64_t tiles_per_block, const uint2* __r
 
 using namespace hepf;
 
-static void sel_geometry(int64_t n_events, int sms, int64_t* n_tiles, int* grid, int64_t* tiles_per_block) {
+// one wave: at most `slots` = SMs x resident blocks per SM blocks, each owning a contiguous range of tiles
+static void sel_geometry(int64_t n_events, int slots, int64_t* n_tiles, int* grid, int64_t* tiles_per_block) {
   *n_tiles = (n_events + SEL_TILE - 1) / SEL_TILE;
-  int64_t g = *n_tiles < (int64_t)sms * 8 ? *n_tiles : (int64_t)sms * 8;
+  int64_t g = *n_tiles < (int64_t)slots ? *n_tiles : (int64_t)slots;
   if (g < 1) g = 1;
   *tiles_per_block = (*n_tiles + g - 1) / g;
   if (*tiles_per_block < 1) *tiles_per_block = 1;
@@ -230,7 +231,12 @@ extern "C" int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_c
   HEPF_CUDA_TRY(cudaGetDevice(&dev));
   HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   int64_t n_tiles, tpb; int grid;
-  sel_geometry(n, sms, &n_tiles, &grid, &tpb);
+  static thread_local int resident = 0;   // blocks of select_eval_kernel that fit on one SM (register-limited)
+  if (!resident) {
+    HEPF_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, select_eval_kernel, SEL_THREADS, 0));
+    if (resident < 1) resident = 1;
+  }
+  sel_geometry(n, sms * resident, &n_tiles, &grid, &tpb);
   if (grid > 4096) { set_error("hepf_select: grid %d exceeds the workspace layout", grid); return HEPF_ERR_CAPACITY; }
   uint2* masks = reinterpret_cast<uint2*>(ws);
   uint32_t* block_count = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(ws) +
