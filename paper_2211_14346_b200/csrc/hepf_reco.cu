@@ -203,10 +203,10 @@ __device__ __forceinline__ float cos_third_acos(float c) {
 
 // Seed for the largest real root of the resolvent cubic m^3 + p m^2 + (p^2/4 - r) m - q^2/8 = 0: the closed form
 // (Cardano / trigonometric) evaluated in FP32 on the FP32 pipe, after an exact power-of-two rescaling t = 2^E tau that
-// brings the depressed quartic's coefficients to O(1).  Only a starting point: FP64 Newton steps follow.
-__device__ __forceinline__ double resolvent_seed(double p, double q, double r) {
-  int E = max(max((exp_of(p) + 1) >> 1, (exp_of(q) + 2) / 3), (exp_of(r) + 3) >> 2);
-  E = min(250, max(-250, E));
+// brings the depressed quartic's coefficients to O(1).  2^E is the scale of the problem, taken from the imposed top mass
+// (the roots are neutrino momenta of that order); a quartic far off that scale over- or underflows FP32, the seed is
+// then useless and the rescue path below takes over, at a cost in speed only.  A starting point: FP64 Newton steps follow.
+__device__ __forceinline__ double resolvent_seed(double p, double q, double r, int E) {
   const float pf = (float)(p * pow2(-2 * E)), qf = (float)(q * pow2(-3 * E)), rf = (float)(r * pow2(-4 * E));
   const float c1 = fmaf(0.25f * pf, pf, -rf), c0 = -0.125f * qf * qf;
   const float p3 = pf * (1.0f / 3.0f);
@@ -227,6 +227,9 @@ __device__ __forceinline__ double resolvent_seed(double p, double q, double r) {
   }
   return (double)(w - p3) * pow2(2 * E);
 }
+
+// exponent of the FP32 seed's scale: 2^E <= m_top < 2^(E+1), clamped so that 2^(+-4E) stays a normal double
+__device__ __forceinline__ int seed_scale(const hepf_tth_params_t& P) { return min(250, max(-250, exp_of(P.m_top))); }
 
 // Largest real root of m^3 + p m^2 + c1 m + c0 (c0 <= 0, so it is >= 0) by Newton from an upper bound of all roots: the
 // iterates decrease monotonically onto it.  Slow path of solve_quartic; NaN coefficients fall through and return NaN.
@@ -271,13 +274,13 @@ __device__ __noinline__ Biquad biquadratic_roots(double p, double r, double aq) 
 
 // Real roots of x^4 + g3 x^3 + g2 x^2 + g1 x + g0 by Ferrari's closed form; the polish happens later, on the pair of
 // conics.  Roots come out as pair A (xa[0], xa[1]) and pair B (xb[0], xb[1]).  Returns bit 0 = pair A real, bit 1 = B.
-__device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, double g0, double (&xa)[2], double (&xb)[2]) {
+__device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, double g0, int seedE, double (&xa)[2], double (&xb)[2]) {
   const double aq = 0.25 * g3, aq2 = aq * aq;
   const double p = fma(-6.0, aq2, g2);
   const double q = fma(aq, fma(8.0, aq2, -2.0 * g2), g1);
   const double r = fma(aq2, fma(-3.0, aq2, g2), fma(-aq, g1, g0));
   const double c1 = fma(0.25 * p, p, -r), c0 = -0.125 * q * q, tp = 2.0 * p;
-  double m = resolvent_seed(p, q, r), step = 0.0;
+  double m = resolvent_seed(p, q, r, seedE), step = 0.0;
 #pragma unroll
   for (int it = 0; it < 2; it++) {   // FP64 Newton on the resolvent cubic
     const double f = fma(fma(m + p, m, c1), m, c0), df = fma(fma(3.0, m, tp), m, c1);
@@ -511,6 +514,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   __syncwarp();
   const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2), inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
   const unsigned lt = (1u << lane) - 1u;
+  const int seedE = seed_scale(P);
   double best_ll = -CUDART_INF;
   uint32_t best_key = 0xffffffffu;
   int qn = 0;                                      // stack height (warp-uniform)
@@ -588,7 +592,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         const PairConst K{W.pc[0][ap], W.pc[1][ap], W.pc[2][ap], W.pc[3][ap]};
         double g3, g2, g1, g0;
         resultant(A, B, K, g3, g2, g1, g0);
-        mask = solve_quartic(g3, g2, g1, g0, xa, xb);
+        mask = solve_quartic(g3, g2, g1, g0, seedE, xa, xb);
         if (mask) {
           double ht; int hh, kk, ll;
           best_higgs<NBT, VC>(&W.ht[vv], nb, i, j, ht, hh, kk, ll);
@@ -720,7 +724,7 @@ reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_id
   const Conic B = shift_conic(q2, Mx, My);
   double g3, g2, g1, g0, xa[2] = {0, 0}, xb[2] = {0, 0};
   resultant(A, B, pair_consts(A.a, A.b, A.c, B.a, B.b, B.c), g3, g2, g1, g0);
-  const int mask = solve_quartic(g3, g2, g1, g0, xa, xb);
+  const int mask = solve_quartic(g3, g2, g1, g0, seed_scale(P), xa, xb);
   double xs[4], ys[4]; int nr = 0;
   if (mask & 1) { xs[0] = xa[0]; xs[1] = xa[1]; nr = 2; }
   if (mask & 2) { xs[nr] = xb[0]; xs[nr + 1] = xb[1]; nr += 2; }
@@ -847,6 +851,7 @@ extern "C" int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t*
   else if (cfg == 165) rc = launch_search_both<16, 2, 11, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   else if (cfg == 166) rc = launch_search_both<16, 1, 22, 14>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   else if (cfg == 164) rc = launch_search_both<16, 4, 5, 3>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  else if (cfg == 167) rc = launch_search_both<16, 2, 10, 8>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   else rc = launch_search_both<16, 2, 10, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   if (rc != HEPF_OK) return rc;
   const int64_t fblocks = (n_idx + 127) / 128;
