@@ -317,3 +317,31 @@ def test_cfg5_full_stream_sampled_windows(hepf):
         got = out[start:start + m].cpu().numpy()
         assert got.tobytes() == oracle.philox_normal(7, start, m).tobytes(), start
     del out
+
+
+def test_other_units_and_off_scale_seed(hepf):
+    """The FP32 seed of the resolvent root is scaled by 2^E with E from m_top; the result must not depend on it.
+    (a) the same events in MeV (every momentum, mass and width x 1000): the seed scale follows m_top;
+    (b) GeV events with a deliberately absurd seed scale is not reachable through the ABI, so instead the masses are
+        left alone and the momenta are scaled by 1/64 with all mass parameters: a different E, same physics."""
+    import parity
+    st = hs.generate(1500, 31, with_truth=False)
+    for scale in (1000.0, 1.0 / 64.0):
+        s2 = hs.EventStore(st.n_events, st.stride, st.event_base, st.cols.copy(), st.flags.copy())
+        for name, r in hs.ROW.items():
+            if name in ("lep_eta", "jet_eta"):
+                continue
+            nrow = 2 if name.startswith("lep") else (8 if name.startswith("jet") else 1)
+            s2.cols[r:r + nrow] *= scale
+        kw = dict(m_top=172.5 * scale, m_w=80.4 * scale, m_higgs=125.0 * scale, sigma_higgs=15.0 * scale,
+                  lambda_nu=40.0 * scale, jet_stoch=0.5 * np.sqrt(scale))
+        chain = [(k, n, lo * scale if k in (hs.LEP_PT_GT, hs.NJET_GE, hs.NBJET_GE, hs.MET_GT, hs.MLL_GT) else lo, hi)
+                 for (k, n, lo, hi) in hs.CHAIN_BASE]
+        dev, idx_t, n, idx, _ = _gpu_select(hepf, s2, chain)
+        assert n > 400
+        got = _gpu_reco(hepf, dev, idx_t, n, 8, 77, hepf.default_params(**kw))
+        Po = oracle.default_params(**kw)
+        want, aux = oracle.reconstruct_tth(s2, idx, 8, 77, Po, n_threads=8)
+        cls, fails = parity.compare(s2, got, want, aux, 8, 77, Po, m_top=172.5 * scale, m_w=80.4 * scale)
+        assert not fails, fails[:5]
+        assert cls["match"] > 0.95 * n
