@@ -32,10 +32,10 @@ UNIT = "reconstructions/s"
 FP64_LANES_PER_SM = 64
 # Algorithmic FP64 work of one solve: the search kernel's own predicated-on thread-level FP64 instruction counts per
 # solve (idle lanes and divergence waste do not count), from the committed ncu capture of this build
-# (profiles/r01d_reco_search.md): DADD + DMUL + DFMA lane-ops, and flop with FMA = 2.  DESIGN.md section 7.
-FP64_OPS_PER_SOLVE = {"dadd": 32.6, "dmul": 81.9, "dfma": 158.2}
-FP64_OPS_PER_SOLVE_NB6 = {"dadd": 26.4, "dmul": 68.1, "dfma": 129.6}   # n_b = 6 kernel (cfg3), profiles/r01d
-DRAM_BYTES_PER_LAUNCH = 276.2e6   # ncu dram__bytes_read.sum + dram__bytes_write.sum of the search kernel (same profile)
+# (profiles/r01e_final.md): DADD + DMUL + DFMA lane-ops, and flop with FMA = 2.  DESIGN.md section 7.
+FP64_OPS_PER_SOLVE = {"dadd": 34.5, "dmul": 78.1, "dfma": 142.9}
+FP64_OPS_PER_SOLVE_NB6 = {"dadd": 27.1, "dmul": 62.9, "dfma": 114.1}   # n_b = 6 kernel (cfg3), profiles/r01e
+DRAM_BYTES_PER_LAUNCH = 275.1e6   # ncu dram__bytes_read.sum + dram__bytes_write.sum of the search kernel (same profile)
 
 
 def chain_bytes_per_event(chain) -> int:
