@@ -482,7 +482,6 @@ template <int VC, int NBT>
 __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const RecoCols& ev, const EventHead& h, int V, uint32_t k0,
                                                  uint32_t k1, const hepf_tth_params_t& P, int lane) {
   constexpr int LPB = 32 / VC;     // item sub-groups per warp pass
-  constexpr int NP = WarpMem<VC, NBT>::NP;
   const int vv = lane & (VC - 1), sub = lane / VC;
   // ---- prologue: nominal objects, kappa*sigma, MET ------------------------------------------------------------------
   if (lane < 10) {
