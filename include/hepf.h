@@ -147,6 +147,23 @@ int hepf_tth_host(const hepf_events_t* host_events, const hepf_cut_t* host_cuts,
                   size_t arena_bytes, void* stream);
 size_t hepf_tth_host_arena_bytes(int64_t n_events, int32_t n_variations);
 
+/*
+ * hepf_histogram — fixed-width histogram of one quantity of the reconstructed events, filled on the device
+ * (App. 8.2: the user's finalize() writes histograms of reconstructed quantities; PAPER.md:278:
+ * per-cut variable recording).  Only records with status bit 0 (has a solution) are filled.
+ *   best    device hepf_best_t[n].
+ *   field   HEPF_H_* below.  NU_PT / NUBAR_PT = sqrt(px*px + py*py), each operation rounded once (no contraction).
+ *   bins    t = (value - lo) * (nbins / (hi - lo)), every operation rounded once; t < 0 -> out[0] (underflow),
+ *           t >= nbins -> out[nbins + 1] (overflow), else out[1 + (int)t]; a NaN value is not counted.
+ *   out     device uint64[nbins + 2], ZEROED by the call before filling; 1 <= nbins <= 4096, hi > lo.
+ */
+typedef enum {
+  HEPF_H_M_TOP = 0, HEPF_H_M_ANTITOP = 1, HEPF_H_M_WPLUS = 2, HEPF_H_M_WMINUS = 3, HEPF_H_M_HIGGS = 4,
+  HEPF_H_LOGLIK = 5, HEPF_H_NU_PT = 6, HEPF_H_NUBAR_PT = 7, HEPF_H_VARIATION = 8
+} hepf_hist_field_t;
+int hepf_histogram(const hepf_best_t* best, int64_t n, int field, double lo, double hi, int32_t nbins, uint64_t* out,
+                   void* stream);
+
 /* Kernel launches enqueued by this thread's calls since the last reset (bench.py's `gpu_launches`). */
 int64_t hepf_launch_count(int reset);
 /* FP64 FMA-chain micro-benchmark used to measure the FP64 roof on the box: enqueues one kernel that performs

@@ -13,7 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libhepf_oracle.so")
-_SRCS = ["oracle_philox.cpp", "oracle_select.cpp", "oracle_reco.cpp"]
+_SRCS = ["oracle_philox.cpp", "oracle_select.cpp", "oracle_reco.cpp", "oracle_hist.cpp"]
 
 
 def build(force: bool = False) -> str:
@@ -78,6 +78,7 @@ def lib():
                                     C.POINTER(Params), C.POINTER(Pairing)]
         L.orc_smear.argtypes = [C.POINTER(Events), C.c_uint32, C.c_int32, C.c_uint64, C.POINTER(Params),
                                 C.c_void_p, C.c_void_p]
+        L.orc_histogram.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
 
@@ -186,3 +187,16 @@ def smear(store, e: int, v: int, seed: int, params: Params | None = None):
     if rc != 0:
         raise RuntimeError(f"orc_smear: {rc}")
     return s, m
+
+
+HIST_FIELDS = dict(m_top=0, m_antitop=1, m_wplus=2, m_wminus=3, m_higgs=4, loglik=5, nu_pt=6, nubar_pt=7, variation=8)
+
+
+def histogram(best: np.ndarray, field: str, lo: float, hi: float, nbins: int) -> np.ndarray:
+    """uint64[nbins + 2]: underflow, bins, overflow of the solved records' `field`."""
+    best = np.ascontiguousarray(best)
+    out = np.zeros(nbins + 2, dtype=np.uint64)
+    rc = lib().orc_histogram(best.ctypes.data, len(best), HIST_FIELDS[field], lo, hi, nbins, out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_histogram: {rc}")
+    return out

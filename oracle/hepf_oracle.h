@@ -21,6 +21,7 @@
  *                              truth recovery in closure mode, multi-start Newton brute force on the
  *                              raw mass constraints, dense-grid sign-change brute force on the quartic
  *   O4 score / argmax ........ prefix property in V, sigma_scale = 0, z-rotation invariance, slot permutation
+ *   histogram ................ hand-built edge cases (lower edge in, upper edge overflow, NaN, unsolved), numpy restatement
  *   PARITY UNPINNED against the paper: the likelihood formula, sigma_H, lambda_nu, the resolution model
  *   and the 8-cut thresholds are definitions of this build (R3, R7, R10), not paper values.
  */
@@ -100,6 +101,9 @@ int orc_eval_cell(const orc_events_t* ev, uint32_t e, int32_t v, int32_t a, uint
 /* smeared objects of one (event, variation): scales[10], met'[2] */
 int orc_smear(const orc_events_t* ev, uint32_t e, int32_t v, uint64_t seed, const orc_params_t* params,
               double scales[10], double metp[2]);
+
+/* histogram of a field of the records (oracle_hist.cpp; pin: numpy restatement + hand-built edge cases) */
+int orc_histogram(const orc_best_t* best, int64_t n, int field, double lo, double hi, int32_t nbins, uint64_t* out);
 
 #ifdef __cplusplus
 }

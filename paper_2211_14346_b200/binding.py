@@ -76,6 +76,7 @@ def load():
         L.hepf_tth_host.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_int32, C.c_uint64,
                                     C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_size_t, C.c_void_p]
+        L.hepf_histogram.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
         L.hepf_timing_enable.argtypes = [C.c_int]
         L.hepf_timing_ms.restype = C.c_double
         L.hepf_timing_ms.argtypes = [C.c_int, C.c_int]
@@ -248,3 +249,17 @@ def timing_enable(on: bool = True):
 def timing_ms(from_slot: int, to_slot: int) -> float:
     """Elapsed device milliseconds between two of the library's timing slots (see include/hepf.h)."""
     return float(load().hepf_timing_ms(from_slot, to_slot))
+
+
+HIST_FIELDS = dict(m_top=0, m_antitop=1, m_wplus=2, m_wminus=3, m_higgs=4, loglik=5, nu_pt=6, nubar_pt=7, variation=8)
+
+
+def histogram(best, n: int, field: str, lo: float, hi: float, nbins: int, *, out=None, stream=None):
+    """hepf_histogram: int64 tensor [nbins + 2] (underflow, bins, overflow) of `field` over the solved records of
+    `best` (the uint8 [n, 128] tensor hepf_reconstruct_tth filled)."""
+    import torch
+    if out is None:
+        out = torch.empty(nbins + 2, dtype=torch.int64, device=best.device)
+    rc = load().hepf_histogram(best.data_ptr(), n, HIST_FIELDS[field], lo, hi, nbins, out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "hepf_histogram")
+    return out

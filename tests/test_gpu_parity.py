@@ -345,3 +345,32 @@ def test_other_units_and_off_scale_seed(hepf):
         cls, fails = parity.compare(s2, got, want, aux, 8, 77, Po, m_top=172.5 * scale, m_w=80.4 * scale)
         assert not fails, fails[:5]
         assert cls["match"] > 0.95 * n
+
+
+# ------------------------------------------------------------------------------------------------------- histogram
+def test_histogram_counts_are_bit_exact(hepf):
+    """hepf_histogram against the oracle: every field, on real records (cfg1) and on planted edge values."""
+    import torch
+    cfg = hs.CONFIGS[1]
+    st = cfg.events()
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, cfg.cuts)
+    rec_t = hepf.reconstruct_tth(dev, idx_t, n, cfg.n_variations, cfg.reco_seed)
+    torch.cuda.synchronize()
+    from paper_2211_14346_b200.binding import best_to_numpy
+    rec = best_to_numpy(rec_t)
+    for field, lo, hi, nb in (("m_higgs", 0.0, 300.0, 60), ("loglik", -10.0, 6.0, 128), ("nu_pt", 0.0, 200.0, 100),
+                              ("nubar_pt", 0.0, 200.0, 4096), ("m_top", 172.0, 173.0, 7), ("m_wminus", 80.3, 80.5, 1),
+                              ("m_antitop", 0.0, 1.0, 3), ("m_wplus", 80.4, 80.400001, 11), ("variation", 0.0, 16.0, 16)):
+        got = hepf.histogram(rec_t, n, field, lo, hi, nb).cpu().numpy().astype(np.uint64)
+        assert np.array_equal(got, oracle.histogram(rec, field, lo, hi, nb)), field
+        assert int(got.sum()) <= int((rec["status"] & 1).sum())
+    planted = np.zeros(3000, dtype=oracle.BEST_DTYPE)
+    rng = np.random.default_rng(2)
+    planted["m_higgs"] = np.concatenate([np.linspace(100.0, 150.0, 1001), rng.uniform(90, 160, 1996), [np.nan, np.inf, -np.inf]])
+    planted["status"] = rng.integers(0, 8, 3000)
+    pt = torch.from_numpy(planted.view(np.uint8).reshape(-1, 128)).cuda()
+    got = hepf.histogram(pt, len(planted), "m_higgs", 100.0, 150.0, 1000).cpu().numpy().astype(np.uint64)
+    assert np.array_equal(got, oracle.histogram(planted, "m_higgs", 100.0, 150.0, 1000))
+    assert np.array_equal(hepf.histogram(pt, 0, "m_higgs", 0.0, 1.0, 5).cpu().numpy(), np.zeros(7, dtype=np.int64))
+    with pytest.raises(hepf.HepfError):
+        hepf.histogram(pt, 10, "m_higgs", 1.0, 1.0, 5)
