@@ -37,7 +37,7 @@ def build(force: bool = False) -> str:
 class _GenCfg(ctypes.Structure):
     _fields_ = [("n_events", ctypes.c_int64), ("first_event", ctypes.c_int64), ("stride", ctypes.c_int64),
                 ("seed", ctypes.c_uint64), ("n_fake_b", ctypes.c_int32), ("closure", ctypes.c_int32),
-                ("bkg_frac", ctypes.c_double)]
+                ("bkg_frac", ctypes.c_double), ("semilep", ctypes.c_int32), ("pad_", ctypes.c_int32)]
 
 
 _lib = None
@@ -79,14 +79,14 @@ class EventStore:
 
 
 def generate(n_events: int, seed: int, *, n_fake_b: int = 0, bkg_frac: float = 0.0, closure: bool = False,
-             first_event: int = 0, with_truth: bool = True) -> EventStore:
+             first_event: int = 0, with_truth: bool = True, semilep: bool = False) -> EventStore:
     lib = _load()
     stride = n_events + (n_events & 1)
     stride = max(stride, 2)
     cols = np.zeros((NROW, stride), dtype=np.float64)
     flags = np.zeros(stride, dtype=np.uint32)
     truth = np.zeros((n_events, 12), dtype=np.float64) if with_truth else None
-    cfg = _GenCfg(n_events, first_event, stride, seed, n_fake_b, int(closure), bkg_frac)
+    cfg = _GenCfg(n_events, first_event, stride, seed, n_fake_b, int(closure), bkg_frac, int(semilep), 0)
     rc = lib.hepf_synth_generate(ctypes.byref(cfg), cols.ctypes.data, flags.ctypes.data,
                                  truth.ctypes.data if truth is not None else None)
     if rc != 0:

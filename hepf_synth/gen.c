@@ -35,6 +35,8 @@ typedef struct {
   int32_t n_fake_b;      /* extra b-tagged fake jets per signal event (0 / 2) */
   int32_t closure;       /* 1: zero widths, no detector smearing, no extras   */
   double bkg_frac;       /* probability of a structure-less background event  */
+  int32_t semilep;       /* 1: semileptonic ttbar events (1 lepton, 2 b + 2 light jets) for the chi2 path */
+  int32_t pad_;
 } hepf_gen_cfg_t;
 
 typedef struct { uint64_t s; } rng_t;
@@ -203,6 +205,49 @@ static void gen_signal(const hepf_gen_cfg_t* c, rng_t* r, double* cols, uint32_t
   write_event(c, cols, flags, truth, k, 2, lep, lq, nj, jets, mx, my, tnu, tnub, 1);
 }
 
+/* Semileptonic ttbar (section 6.2): t -> W b, W -> l nu; tbar -> W bbar, W -> q qbar'.  One lepton,
+ * two b-tagged and two untagged jets (+ 0-2 extra untagged light jets), MET = neutrino pT.  Truth: nu[3], nubar unused (0),
+ * slots of b_lep, b_had, q1, q2. */
+static void gen_semilep(const hepf_gen_cfg_t* c, rng_t* r, double* cols, uint32_t* flags, double* truth, int64_t k) {
+  const double MB = 4.7;
+  double mt, mtb, mwp, mwm;
+  if (c->closure) { mt = mtb = 172.5; mwp = mwm = 80.4; }
+  else {
+    mt = rng_bw(r, 172.5, 1.4, 150.0, 195.0); mtb = rng_bw(r, 172.5, 1.4, 150.0, 195.0);
+    mwp = rng_bw(r, 80.4, 2.1, 60.0, 100.0); mwm = rng_bw(r, 80.4, 2.1, 60.0, 100.0);
+  }
+  double M = mt + mtb + rng_exp(r, 120.0);
+  double spt = rng_exp(r, 40.0), sphi = 2.0 * PI * rng_u(r), sy = 1.2 * rng_norm(r);
+  double mT = sqrt(M * M + spt * spt);
+  v4 S = {spt * cos(sphi), spt * sin(sphi), mT * sinh(sy), mT * cosh(sy)};
+  v4 t, tb, wp, b, wm, bb, lp, nu, q1, q2;
+  decay2(r, S, M, mt, mtb, &t, &tb);
+  decay2(r, t, mt, mwp, MB, &wp, &b);
+  decay2(r, wp, mwp, 0.0, 0.0, &lp, &nu);
+  decay2(r, tb, mtb, mwm, MB, &wm, &bb);
+  decay2(r, wm, mwm, 0.0, 0.0, &q1, &q2);
+  lp.e = sqrt(lp.x * lp.x + lp.y * lp.y + lp.z * lp.z);
+  v4 lep[2] = {lp, lp}; int lq[2] = {rng_u(r) < 0.5 ? +1 : -1, 0};
+  jet_t jets[NJ]; int nj = 0;
+  v4 bj[4] = {b, bb, q1, q2};
+  for (int i = 0; i < 4; i++) { jets[nj].p = bj[i]; jets[nj].tag = i < 2; jets[nj].role = i; nj++; }
+  double mx = nu.x, my = nu.y;
+  if (!c->closure) {
+    lep[0] = v4_scale(lep[0], 1.0 + 0.01 * rng_norm(r));
+    for (int i = 0; i < 4; i++) {
+      double s = 1.0 + (0.5 / sqrt(jets[i].p.e) + 0.03) * rng_norm(r);
+      jets[i].p = v4_scale(jets[i].p, s < 0.1 ? 0.1 : s);
+    }
+    int nl = rng_poisson(r, 0.7); if (nl > 2) nl = 2;
+    for (int i = 0; i < nl; i++) {
+      double pt = rng_exp(r, 40.0), eta = 5.0 * rng_u(r) - 2.5, phi = 2.0 * PI * rng_u(r);
+      jets[nj].p = v4_ptetaphim(pt, eta, phi, 0.0); jets[nj].tag = 0; jets[nj].role = -1; nj++;
+    }
+  }
+  double tnu[3] = {nu.x, nu.y, nu.z}, z3[3] = {0, 0, 0};
+  write_event(c, cols, flags, truth, k, 1, lep, lq, nj, jets, mx, my, tnu, z3, 1);
+}
+
 static void gen_background(const hepf_gen_cfg_t* c, rng_t* r, double* cols, uint32_t* flags, double* truth, int64_t k) {
   double u = rng_u(r);
   int n_lep = u < 0.2 ? 1 : (u < 0.9 ? 2 : 3);
@@ -228,7 +273,8 @@ int hepf_synth_generate(const hepf_gen_cfg_t* c, double* cols, uint32_t* flags, 
 #pragma omp parallel for schedule(static)
   for (int64_t k = 0; k < c->n_events; k++) {
     rng_t r; rng_init(&r, c->seed, (uint64_t)(c->first_event + k));
-    if (c->bkg_frac > 0.0 && rng_u(&r) < c->bkg_frac) gen_background(c, &r, cols, flags, truth, k);
+    if (c->semilep) gen_semilep(c, &r, cols, flags, truth, k);
+    else if (c->bkg_frac > 0.0 && rng_u(&r) < c->bkg_frac) gen_background(c, &r, cols, flags, truth, k);
     else gen_signal(c, &r, cols, flags, truth, k);
   }
   return 0;

@@ -13,7 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libhepf_oracle.so")
-_SRCS = ["oracle_philox.cpp", "oracle_select.cpp", "oracle_reco.cpp", "oracle_hist.cpp"]
+_SRCS = ["oracle_philox.cpp", "oracle_select.cpp", "oracle_reco.cpp", "oracle_hist.cpp", "oracle_chi2.cpp"]
 
 
 def build(force: bool = False) -> str:
@@ -78,6 +78,8 @@ def lib():
                                     C.POINTER(Params), C.POINTER(Pairing)]
         L.orc_smear.argtypes = [C.POINTER(Events), C.c_uint32, C.c_int32, C.c_uint64, C.POINTER(Params),
                                 C.c_void_p, C.c_void_p]
+        L.orc_nu_pz.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_void_p]
+        L.orc_chi2_semilep.argtypes = [C.POINTER(Events), C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_histogram.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
@@ -200,3 +202,28 @@ def histogram(best: np.ndarray, field: str, lo: float, hi: float, nbins: int) ->
     if rc != 0:
         raise RuntimeError(f"orc_histogram: {rc}")
     return out
+
+
+CHI2_DTYPE = np.dtype([("chi2", "f8"), ("nu_pz", "f8"), ("m_top_lep", "f8"), ("m_top_had", "f8"), ("m_w_lep", "f8"),
+                       ("m_w_had", "f8"), ("jet_b_lep", "i4"), ("jet_b_had", "i4"), ("jet_q1", "i4"), ("jet_q2", "i4"),
+                       ("solution", "i4"), ("n_comb", "i4"), ("status", "u4"), ("event", "u4")])
+assert CHI2_DTYPE.itemsize == 80
+
+
+def nu_pz(lep, nux: float, nuy: float, m_w: float = 80.4):
+    lep = np.ascontiguousarray(lep, dtype=np.float64); pz = np.zeros(2)
+    n = lib().orc_nu_pz(lep.ctypes.data, nux, nuy, m_w, pz.ctypes.data)
+    return list(pz[:n])
+
+
+def chi2_semilep(store, idx, params=None):
+    """(records CHI2_DTYPE[n], second-best chi2 per event); params = (m_top, m_w, sigma_top, sigma_w) or None."""
+    ev = events_view(store)
+    idx = np.ascontiguousarray(idx, dtype=np.uint32)
+    out = np.zeros(len(idx), dtype=CHI2_DTYPE); second = np.zeros(len(idx))
+    par = np.asarray(params, dtype=np.float64) if params is not None else None
+    rc = lib().orc_chi2_semilep(C.byref(ev), idx.ctypes.data, len(idx), par.ctypes.data if par is not None else None,
+                                out.ctypes.data, second.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_chi2_semilep: {rc}")
+    return out, second

@@ -21,6 +21,8 @@
  *                              truth recovery in closure mode, multi-start Newton brute force on the
  *                              raw mass constraints, dense-grid sign-change brute force on the quartic
  *   O4 score / argmax ........ prefix property in V, sigma_scale = 0, z-rotation invariance, slot permutation
+ *   chi2 (semileptonic) ...... p_z against a dense scan of m(l nu), truth recovery in closure mode (chi2 = 0 at the true
+ *                              combination), brute-force enumeration in numpy, permutation invariance
  *   histogram ................ hand-built edge cases (lower edge in, upper edge overflow, NaN, unsolved), numpy restatement
  *   PARITY UNPINNED against the paper: the likelihood formula, sigma_H, lambda_nu, the resolution model
  *   and the 8-cut thresholds are definitions of this build (R3, R7, R10), not paper values.
@@ -101,6 +103,18 @@ int orc_eval_cell(const orc_events_t* ev, uint32_t e, int32_t v, int32_t a, uint
 /* smeared objects of one (event, variation): scales[10], met'[2] */
 int orc_smear(const orc_events_t* ev, uint32_t e, int32_t v, uint64_t seed, const orc_params_t* params,
               double scales[10], double metp[2]);
+
+/* chi^2 reconstruction of semileptonic ttbar (eq. 1; oracle_chi2.cpp) */
+typedef struct { double m_top, m_w, sigma_top, sigma_w; } orc_chi2_params_t;
+typedef struct {
+  double chi2, nu_pz, m_top_lep, m_top_had, m_w_lep, m_w_had;
+  int32_t jet_b_lep, jet_b_had, jet_q1, jet_q2, solution, n_comb;
+  uint32_t status, event;
+} orc_chi2_t;   /* 80 bytes */
+void orc_default_chi2_params(orc_chi2_params_t* p);
+int orc_nu_pz(const double lep[4], double nux, double nuy, double m_w, double pz[2]);
+int orc_chi2_semilep(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx, const orc_chi2_params_t* params,
+                     orc_chi2_t* out, double* out_second);
 
 /* histogram of a field of the records (oracle_hist.cpp; pin: numpy restatement + hand-built edge cases) */
 int orc_histogram(const orc_best_t* best, int64_t n, int field, double lo, double hi, int32_t nbins, uint64_t* out);
