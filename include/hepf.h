@@ -148,6 +148,26 @@ int hepf_tth_host(const hepf_events_t* host_events, const hepf_cut_t* host_cuts,
 size_t hepf_tth_host_arena_bytes(int64_t n_events, int32_t n_variations);
 
 /*
+ * hepf_chi2_semilep — chi^2 kinematic reconstruction of semileptonic ttbar events (section 6.2, eq. 1;
+ * SURVEY.md 8(f) NEXT-2):  chi^2 = ((m_blnu - m_t)/sigma_t)^2 + ((m_lnu - m_W)/sigma_W)^2 + ((m_bjj - m_t)/sigma_t)^2 +
+ * ((m_jj - m_W)/sigma_W)^2, minimised over the combinations (b_lep, b_had: ordered pair of the first 4 b-tagged jet slots;
+ * q1 < q2: pair of the first 4 untagged slots) and over the neutrino p_z: pT(nu) = MET, p_z solves m(l nu) = m_W (two
+ * solutions, index 0 = smaller p_z) or, without a real solution, minimises m(l nu) (R14).  Argmin in the order
+ * (b_lep, b_had, (q1, q2), solution), strict <.
+ *   idx          device uint32[n_idx] events to reconstruct;  host_params NULL = (172.5, 80.4, 11.5, 7.5).
+ *   out          device hepf_chi2_t[n_idx], 16-byte aligned.  status 1 = reconstructed, 2 = not applicable (n_lep != 1,
+ *                fewer than 2 b-tagged or fewer than 2 untagged jets): NaN / -1 payload.
+ */
+typedef struct { double m_top, m_w, sigma_top, sigma_w; } hepf_chi2_params_t;
+typedef struct {
+  double chi2, nu_pz, m_top_lep, m_top_had, m_w_lep, m_w_had;
+  int32_t jet_b_lep, jet_b_had, jet_q1, jet_q2, solution, n_comb;
+  uint32_t status, event;
+} hepf_chi2_t;   /* 80 bytes */
+int hepf_chi2_semilep(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, const hepf_chi2_params_t* host_params,
+                      hepf_chi2_t* out, void* stream);
+
+/*
  * hepf_histogram — fixed-width histogram of one quantity of the reconstructed events, filled on the device
  * (App. 8.2: the user's finalize() writes histograms of reconstructed quantities; PAPER.md:278:
  * per-cut variable recording).  Only records with status bit 0 (has a solution) are filled.

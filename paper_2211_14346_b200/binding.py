@@ -76,6 +76,7 @@ def load():
         L.hepf_tth_host.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_int32, C.c_uint64,
                                     C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_size_t, C.c_void_p]
+        L.hepf_chi2_semilep.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.hepf_histogram.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
         L.hepf_timing_enable.argtypes = [C.c_int]
         L.hepf_timing_ms.restype = C.c_double
@@ -263,3 +264,22 @@ def histogram(best, n: int, field: str, lo: float, hi: float, nbins: int, *, out
     rc = load().hepf_histogram(best.data_ptr(), n, HIST_FIELDS[field], lo, hi, nbins, out.data_ptr(), _stream_ptr(stream))
     _check(rc, "hepf_histogram")
     return out
+
+
+CHI2_DTYPE = np.dtype([("chi2", "f8"), ("nu_pz", "f8"), ("m_top_lep", "f8"), ("m_top_had", "f8"), ("m_w_lep", "f8"),
+                       ("m_w_had", "f8"), ("jet_b_lep", "i4"), ("jet_b_had", "i4"), ("jet_q1", "i4"), ("jet_q2", "i4"),
+                       ("solution", "i4"), ("n_comb", "i4"), ("status", "u4"), ("event", "u4")])
+assert CHI2_DTYPE.itemsize == 80
+
+
+def chi2_semilep(events: DeviceEvents, idx, n_idx: int, params=None, *, out=None, stream=None):
+    """hepf_chi2_semilep: uint8 tensor [n_idx, 80] of hepf_chi2_t records (see CHI2_DTYPE); params = (m_top, m_w,
+    sigma_top, sigma_w) or None for the paper's values."""
+    import torch
+    if out is None:
+        out = torch.empty((max(n_idx, 1), 80), dtype=torch.uint8, device=events.cols.device)
+    ev = events.view()
+    par = (C.c_double * 4)(*params) if params is not None else None
+    rc = load().hepf_chi2_semilep(C.byref(ev), idx.data_ptr(), n_idx, par, out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "hepf_chi2_semilep")
+    return out[:n_idx]

@@ -374,3 +374,50 @@ def test_histogram_counts_are_bit_exact(hepf):
     assert np.array_equal(hepf.histogram(pt, 0, "m_higgs", 0.0, 1.0, 5).cpu().numpy(), np.zeros(7, dtype=np.int64))
     with pytest.raises(hepf.HepfError):
         hepf.histogram(pt, 10, "m_higgs", 1.0, 1.0, 5)
+
+
+# ------------------------------------------------------------------------------------- chi^2 (semileptonic ttbar)
+def _chi2_compare(got, want, second):
+    assert np.array_equal(got["event"], want["event"]) and np.array_equal(got["status"], want["status"])
+    assert np.array_equal(got["n_comb"], want["n_comb"])
+    ok = want["status"] == 1
+    assert np.isnan(got["chi2"][~ok]).all() and (got["jet_b_lep"][~ok] == -1).all()
+    rel = np.abs(got["chi2"][ok] - want["chi2"][ok]) / np.maximum(1.0, np.abs(want["chi2"][ok]))
+    assert rel.max() <= 1e-9
+    keys = ("jet_b_lep", "jet_b_had", "jet_q1", "jet_q2", "solution")
+    same = np.all([got[k][ok] == want[k][ok] for k in keys], axis=0)
+    tie = (second[ok] - want["chi2"][ok]) <= 1e-9 * np.maximum(1.0, np.abs(want["chi2"][ok]))   # north_star's near-tie rule
+    assert (same | tie).all()
+    for f in ("nu_pz", "m_top_lep", "m_top_had", "m_w_lep", "m_w_had"):
+        g, w = got[f][ok][same], want[f][ok][same]
+        assert (np.abs(g - w) <= 1e-9 * np.maximum(1.0, np.abs(w))).all(), f
+    return int(same.sum()), int(ok.sum())
+
+
+def test_chi2_semilep_parity(hepf):
+    import torch
+    from paper_2211_14346_b200.binding import CHI2_DTYPE
+    for n, seed, closure in ((20_001, 41, False), (3000, 42, True)):
+        st = hs.generate(n, seed, semilep=True, closure=closure, with_truth=False)
+        dev = hepf.DeviceEvents.from_host(st)
+        idx = np.arange(n, dtype=np.uint32)
+        idx_t = torch.from_numpy(idx.view(np.int32)).cuda()
+        got = hepf.chi2_semilep(dev, idx_t, n).cpu().numpy().reshape(-1).view(CHI2_DTYPE)
+        want, second = oracle.chi2_semilep(st, idx)
+        same, ok = _chi2_compare(got, want, second)
+        assert ok == n and same >= ok - 2
+    # mixed sample (dileptonic events are "not applicable"), a strided list, other parameters, empty list
+    mix = hs.generate(4000, 43, with_truth=False)
+    sl = hs.generate(4000, 44, semilep=True, with_truth=False)
+    mix.cols[:, 1::2] = sl.cols[:, 1::2]; mix.flags[1::2] = sl.flags[1::2]
+    dev = hepf.DeviceEvents.from_host(mix)
+    idx = np.arange(3, 4000, 3, dtype=np.uint32)
+    idx_t = torch.from_numpy(idx.view(np.int32)).cuda()
+    par = (170.0, 81.0, 9.0, 6.0)
+    got = hepf.chi2_semilep(dev, idx_t, len(idx), par).cpu().numpy().reshape(-1).view(CHI2_DTYPE)
+    want, second = oracle.chi2_semilep(mix, idx, par)
+    same, ok = _chi2_compare(got, want, second)
+    assert 0 < ok < len(idx)
+    assert hepf.chi2_semilep(dev, idx_t, 0).shape[0] == 0
+    with pytest.raises(hepf.HepfError):
+        hepf.chi2_semilep(dev, idx_t, 5, (172.5, 80.4, 0.0, 7.5))
