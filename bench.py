@@ -83,6 +83,44 @@ def run_philox(args):
                                    "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy, read+write)" if peaks else "fallback 6650"}}))
 
 
+def run_chi2(args):
+    """--workload chi2: hepf_chi2_semilep (eq. 1) on synthetic semileptonic ttbar events."""
+    import torch
+    import paper_2211_14346_b200 as hepf
+    hepf.load()
+    torch.cuda.set_device(0)
+    n = args.events or 4_000_000
+    st = hs.generate(n, 11, semilep=True, with_truth=False)
+    dev = hepf.DeviceEvents.from_host(st)
+    idx_t = torch.arange(n, dtype=torch.int32, device="cuda")
+    out = torch.empty((n, 80), dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+    for _ in range(max(3, args.warmup)):
+        hepf.chi2_semilep(dev, idx_t, n, out=out, stream=stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        hepf.chi2_semilep(dev, idx_t, n, out=out, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    f = st.flags[:n].astype(np.int64); nj = np.minimum((f >> 8) & 15, 8)
+    # algorithmic bytes: idx 4 + flags 4 + lepton 32 + MET 16 + 32 per jet that is a candidate (<= 4 tagged + <= 4 untagged) + 80 out
+    by = float((4 + 4 + 32 + 16 + 80) * n + 32 * nj.sum())
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    hbm = float(json.load(open(peaks_path)).get("hbm_gbs", 6650.0)) if os.path.exists(peaks_path) else 6650.0
+    gbs = by / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "chi2-reconstructed semileptonic ttbar events/sec", "value": n / (ms * 1e-3), "unit": "events/s",
+                      "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": True,
+                      "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": f"chi2: {n} semileptonic ttbar events (2 b + 2-4 untagged jets)",
+                                 "l2": f"{by / 1e6:.0f} MB touched per step, larger than L2"},
+                      "gpu_launches": args.steps,
+                      "roofline": {"bound": "hbm", "kernel": "chi2_semilep_kernel", "achieved": gbs, "peak": hbm, "unit": "GB/s",
+                                   "frac": gbs / hbm, "traffic": None, "algorithmic_bytes": by}}))
+
+
 def solves_of(store, idx, n_variations: int) -> int:
     """event x variation x pairing count of the listed events (A = n_b (n_b - 1) for applicable events)."""
     f = store.flags[idx].astype(np.int64)
@@ -192,7 +230,7 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="hepf", choices=["hepf", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "chi2"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--variations", type=int, default=0, help="override the workload's V (SURVEY 8(f) NEXT-1: 128 = ttH_scinp, 1024 = ttH_sci)")
@@ -200,6 +238,8 @@ def main():
     args = ap.parse_args()
     if args.workload == "cfg5":
         return run_philox(args)
+    if args.workload == "chi2":
+        return run_chi2(args)
     cfg = hs.CONFIGS[int(args.workload[3])]
     if args.impl == "reference":
         return run_reference(args, cfg, args.workload)

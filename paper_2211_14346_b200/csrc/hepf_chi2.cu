@@ -6,7 +6,7 @@
 // light-jet pairs, then min over the ordered pairs i != j of L[i] + H[j] — 8 + 24 mass evaluations instead of 144 (rounding is
 // monotone, so the value is the same as the plain enumeration's; the argmin can differ from it only between exactly tied
 // sums).  FP64 with IEEE division and square root; a few hundred FP64 instructions and ~300 bytes per event: the kernel is
-// short and HBM/latency-bound.
+// short; masses use the branch-free sqrt/rcp of hepf_common.cuh (<= 1 ulp), the p_z quadratic keeps IEEE sqrt and division.
 #include <math_constants.h>
 
 #include "hepf_common.cuh"
@@ -24,7 +24,7 @@ struct P4 { double x, y, z, e; };
 __device__ __forceinline__ P4 add4(const P4& a, const P4& b) { return P4{a.x + b.x, a.y + b.y, a.z + b.z, a.e + b.e}; }
 __device__ __forceinline__ double mass4(const P4& a) {
   const double m2 = a.e * a.e - (a.x * a.x + a.y * a.y + a.z * a.z);
-  return sqrt(m2 > 0.0 ? m2 : 0.0);
+  return sqrt_fast(m2 > 0.0 ? m2 : 0.0);
 }
 
 __global__ void __launch_bounds__(C2_THREADS)
@@ -54,6 +54,7 @@ chi2_semilep_kernel(Chi2Cols ev, const uint32_t* __restrict__ idx, int64_t n_idx
     const double mu = (P.m_w * P.m_w - ml2) / 2.0 + (lep.x * nux + lep.y * nuy);
     const double a = lep.e * lep.e - lep.z * lep.z, pt2 = nux * nux + nuy * nuy;
     const double disc = mu * mu * lep.z * lep.z - a * (lep.e * lep.e * pt2 - mu * mu);
+    const double ist = rcp_fast(P.sigma_top), isw = rcp_fast(P.sigma_w);
     double pz[2]; int nsol;
     if (mu > 0.0 && disc >= 0.0) { const double sq = sqrt(disc); pz[0] = (mu * lep.z - sq) / a; pz[1] = (mu * lep.z + sq) / a; nsol = 2; }
     else { pz[0] = sqrt(pt2) * lep.z / sqrt(a); pz[1] = pz[0]; nsol = 1; }
@@ -61,14 +62,14 @@ chi2_semilep_kernel(Chi2Cols ev, const uint32_t* __restrict__ idx, int64_t n_idx
     double L[4], Lmt[4], Lmw[2]; int Ls[4];
     P4 wl[2];
     for (int s = 0; s < nsol; s++) {
-      const P4 nu{nux, nuy, pz[s], sqrt(pt2 + pz[s] * pz[s])};
+      const P4 nu{nux, nuy, pz[s], sqrt_fast(pt2 + pz[s] * pz[s])};
       wl[s] = add4(lep, nu); Lmw[s] = mass4(wl[s]);
     }
     for (int i = 0; i < nbt; i++) {
       L[i] = CUDART_INF; Ls[i] = 0; Lmt[i] = 0.0;
       for (int s = 0; s < nsol; s++) {
         const double mt = mass4(add4(wl[s], bj[i]));
-        const double t1 = (mt - P.m_top) / P.sigma_top, t2 = (Lmw[s] - P.m_w) / P.sigma_w;
+        const double t1 = (mt - P.m_top) * ist, t2 = (Lmw[s] - P.m_w) * isw;
         const double v = t1 * t1 + t2 * t2;
         if (v < L[i]) { L[i] = v; Ls[i] = s; Lmt[i] = mt; }
       }
@@ -78,9 +79,9 @@ chi2_semilep_kernel(Chi2Cols ev, const uint32_t* __restrict__ idx, int64_t n_idx
     for (int j = 0; j < nbt; j++) { H[j] = CUDART_INF; Ha[j] = 0; Hb[j] = 1; Hmt[j] = Hmw[j] = 0.0; }
     for (int qa = 0; qa < nlt; qa++) for (int qb = qa + 1; qb < nlt; qb++) {
       const P4 wh = add4(lj[qa], lj[qb]);
-      const double mw = mass4(wh), t4 = (mw - P.m_w) / P.sigma_w;
+      const double mw = mass4(wh), t4 = (mw - P.m_w) * isw;
       for (int j = 0; j < nbt; j++) {
-        const double mt = mass4(add4(wh, bj[j])), t3 = (mt - P.m_top) / P.sigma_top;
+        const double mt = mass4(add4(wh, bj[j])), t3 = (mt - P.m_top) * ist;
         const double v = t3 * t3 + t4 * t4;
         if (v < H[j]) { H[j] = v; Ha[j] = qa; Hb[j] = qb; Hmt[j] = mt; Hmw[j] = mw; }
       }
