@@ -136,7 +136,9 @@ int hepf_philox_normal(uint64_t seed, uint64_t counter, uint64_t n, double* out,
 /*
  * hepf_tth_host — the whole path from HOST buffers: copies the columns of `host_events` (a view of HOST
  * memory, pinned for full speed) to the device arena, runs hepf_select and hepf_reconstruct_tth and copies the
- * results back.  Synchronous: returns when host_out_* are filled.
+ * results back.  Large samples are cut into up to 8 chunks of consecutive events whose copies (two internal copy
+ * streams) overlap the kernels of the neighbouring chunks; the results are byte-identical to the device entry points
+ * on one view.  Synchronous: returns when host_out_* are filled.
  *   host_out_idx   host uint32[n_events] or NULL;  host_out_best  host hepf_best_t[n_events] (first n_sel used);
  *   host_out_count host int64;  host_out_cutflow host int64[n_cuts] or NULL.
  *   arena          device scratch >= hepf_tth_host_arena_bytes(n_events, n_variations), 256-byte aligned.

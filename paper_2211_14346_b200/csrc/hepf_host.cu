@@ -1,16 +1,24 @@
-// hepf_host.cu — hepf_tth_host: the whole path from HOST buffers (the end-to-end entry point bench.py's `e2e`
-// number goes through): H2D of the event columns -> hepf_select -> hepf_reconstruct_tth -> D2H of the results.
-// Device memory comes from the caller's arena; nothing is allocated here.
+// hepf_host.cu — hepf_tth_host: the whole path from HOST buffers (the end-to-end entry point bench.py's `e2e` number
+// goes through).  Device memory comes from the caller's arena; nothing is allocated here except, once per host thread,
+// two copy streams and a few events.
+//
+// The sample is cut into up to 8 chunks of consecutive events and pipelined: every chunk's columns go host -> device on a
+// copy-in stream (all enqueued up front), the compute stream waits for chunk c's columns, runs hepf_select and the
+// reconstruction on the chunk VIEW (same pointers + offset, event_base + offset: the smearing stream is keyed by the
+// global event index, so the records are bit-identical to a single-view run), and the chunk's survivors and records go
+// device -> host on a copy-out stream while the next chunk computes.  With 516 B/event in and a reconstruction of about
+// the same duration as the copy, the copies hide behind the kernels.
 #include "hepf_common.cuh"
 
 using namespace hepf;
 
 namespace {
+constexpr int MAX_CHUNKS = 8;
+constexpr int64_t MIN_CHUNK = 32768;      // events; smaller samples are not worth splitting
+
 size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 
-struct ArenaLayout {
-  size_t cols, flags, idx, count, cutflow, sel_ws, reco_ws, best, total;
-};
+struct ArenaLayout { size_t cols, flags, idx, count, cutflow, sel_ws, reco_ws, best, total; };
 
 ArenaLayout layout(int64_t n, int64_t stride) {
   ArenaLayout L{};
@@ -18,21 +26,46 @@ ArenaLayout layout(int64_t n, int64_t stride) {
   L.cols = off; off += up256((size_t)64 * stride * sizeof(double));
   L.flags = off; off += up256((size_t)stride * sizeof(uint32_t));
   L.idx = off; off += up256((size_t)(n > 0 ? n : 1) * sizeof(uint32_t));
-  L.count = off; off += 256;
-  L.cutflow = off; off += up256(HEPF_MAX_CUTS * sizeof(int64_t));
+  L.count = off; off += 256;                                             // one int64 per chunk
+  L.cutflow = off; off += up256((size_t)MAX_CHUNKS * HEPF_MAX_CUTS * sizeof(int64_t));
   L.sel_ws = off; off += up256(hepf_select_workspace_bytes(n));
   L.reco_ws = off; off += up256(hepf_reconstruct_workspace_bytes(n, 1));
   L.best = off; off += up256((size_t)(n > 0 ? n : 1) * sizeof(hepf_best_t));
   L.total = off;
   return L;
 }
+
+struct Pipe {                    // per host thread, created on first use
+  cudaStream_t in = nullptr, out = nullptr;
+  cudaEvent_t arrived[MAX_CHUNKS] = {}, done[MAX_CHUNKS] = {}, start = nullptr;
+  bool ok = false;
+};
+thread_local Pipe g_pipe;
+
+int pipe_init() {
+  if (g_pipe.ok) return HEPF_OK;
+  HEPF_CUDA_TRY(cudaStreamCreateWithFlags(&g_pipe.in, cudaStreamNonBlocking));
+  HEPF_CUDA_TRY(cudaStreamCreateWithFlags(&g_pipe.out, cudaStreamNonBlocking));
+  HEPF_CUDA_TRY(cudaEventCreateWithFlags(&g_pipe.start, cudaEventDisableTiming));
+  for (int c = 0; c < MAX_CHUNKS; c++) {
+    HEPF_CUDA_TRY(cudaEventCreateWithFlags(&g_pipe.arrived[c], cudaEventDisableTiming));
+    HEPF_CUDA_TRY(cudaEventCreateWithFlags(&g_pipe.done[c], cudaEventDisableTiming));
+  }
+  g_pipe.ok = true;
+  return HEPF_OK;
+}
+
+__global__ void add_offset_kernel(uint32_t* idx, int64_t n, uint32_t off) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) idx[i] += off;
+}
 }  // namespace
 
 extern "C" size_t hepf_tth_host_arena_bytes(int64_t n_events, int32_t n_variations) {
   (void)n_variations;
   if (n_events < 0) return 0;
-  const int64_t stride = n_events + (n_events & 1);
-  return layout(n_events, stride < 2 ? 2 : stride).total + 256;
+  int64_t stride = (n_events + 3) / 4 * 4; if (stride < 4) stride = 4;
+  return layout(n_events, stride).total + 256;
 }
 
 extern "C" int hepf_tth_host(const hepf_events_t* hev, const hepf_cut_t* host_cuts, int n_cuts, int32_t n_variations,
@@ -43,61 +76,90 @@ extern "C" int hepf_tth_host(const hepf_events_t* hev, const hepf_cut_t* host_cu
   int rc = check_events(hev);
   if (rc != HEPF_OK) return rc;
   if (!host_out_count || (hev->n_events > 0 && !host_out_best)) { set_error("hepf_tth_host: NULL output"); return HEPF_ERR_ARG; }
+  if (n_cuts < 0 || n_cuts > HEPF_MAX_CUTS) { set_error("hepf_tth_host: n_cuts must be 0..%d", HEPF_MAX_CUTS); return HEPF_ERR_ARG; }
   const int64_t n = hev->n_events;
-  int64_t dstride = n + (n & 1); if (dstride < 2) dstride = 2;
+  int64_t dstride = (n + 3) / 4 * 4; if (dstride < 4) dstride = 4;
   const ArenaLayout L = layout(n, dstride);
   if (!arena || !aligned(arena, 256) || arena_bytes < L.total) {
     set_error("hepf_tth_host: arena too small or misaligned (%zu < %zu)", arena_bytes, L.total); return HEPF_ERR_CAPACITY;
   }
+  rc = pipe_init();
+  if (rc != HEPF_OK) return rc;
   char* base = reinterpret_cast<char*>(arena);
   double* dcols = reinterpret_cast<double*>(base + L.cols);
   uint32_t* dflags = reinterpret_cast<uint32_t*>(base + L.flags);
-  // device view with a dense stride; copy each column block row by row (host stride may differ)
-  hepf_events_t dev = *hev;
-  dev.stride = dstride;
-  struct Blk { const double* src; const double** dst; int rows; };
-  const Blk blks[] = {{hev->lep_px, &dev.lep_px, 2}, {hev->lep_py, &dev.lep_py, 2}, {hev->lep_pz, &dev.lep_pz, 2},
-                      {hev->lep_e, &dev.lep_e, 2}, {hev->lep_pt, &dev.lep_pt, 2}, {hev->lep_eta, &dev.lep_eta, 2},
-                      {hev->jet_px, &dev.jet_px, 8}, {hev->jet_py, &dev.jet_py, 8}, {hev->jet_pz, &dev.jet_pz, 8},
-                      {hev->jet_e, &dev.jet_e, 8}, {hev->jet_pt, &dev.jet_pt, 8}, {hev->jet_eta, &dev.jet_eta, 8},
-                      {hev->met_x, &dev.met_x, 1}, {hev->met_y, &dev.met_y, 1}, {hev->met, &dev.met, 1},
-                      {hev->mll, &dev.mll, 1}};
-  int64_t row = 0;
-  for (const Blk& b : blks) {
-    double* d = dcols + row * dstride;
-    *b.dst = d;
-    if (n > 0) {
-      if (hev->stride == dstride) {
-        HEPF_CUDA_TRY(cudaMemcpyAsync(d, b.src, (size_t)b.rows * dstride * sizeof(double), cudaMemcpyHostToDevice, stream));
-      } else {
-        HEPF_CUDA_TRY(cudaMemcpy2DAsync(d, dstride * sizeof(double), b.src, hev->stride * sizeof(double),
-                                        (size_t)n * sizeof(double), b.rows, cudaMemcpyHostToDevice, stream));
-      }
-    }
-    row += b.rows;
-  }
-  dev.flags = dflags;
-  if (n > 0) HEPF_CUDA_TRY(cudaMemcpyAsync(dflags, hev->flags, (size_t)n * sizeof(uint32_t), cudaMemcpyHostToDevice, stream));
   uint32_t* didx = reinterpret_cast<uint32_t*>(base + L.idx);
   int64_t* dcount = reinterpret_cast<int64_t*>(base + L.count);
   int64_t* dcutflow = reinterpret_cast<int64_t*>(base + L.cutflow);
   hepf_best_t* dbest = reinterpret_cast<hepf_best_t*>(base + L.best);
-  rc = hepf_select(&dev, host_cuts, n_cuts, didx, dcount, host_out_cutflow ? dcutflow : nullptr, base + L.sel_ws,
-                   up256(hepf_select_workspace_bytes(n)), stream);
-  if (rc != HEPF_OK) return rc;
-  HEPF_CUDA_TRY(cudaMemcpyAsync(host_out_count, dcount, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
-  HEPF_CUDA_TRY(cudaStreamSynchronize(stream));
-  const int64_t n_sel = *host_out_count;
-  rc = hepf_reconstruct_tth(&dev, didx, n_sel, n_variations, seed, host_params, dbest, base + L.reco_ws,
-                            up256(hepf_reconstruct_workspace_bytes(n, 1)), stream);
-  if (rc != HEPF_OK) return rc;
-  if (n_sel > 0) {
-    HEPF_CUDA_TRY(cudaMemcpyAsync(host_out_best, dbest, (size_t)n_sel * sizeof(hepf_best_t), cudaMemcpyDeviceToHost, stream));
-    if (host_out_idx)
-      HEPF_CUDA_TRY(cudaMemcpyAsync(host_out_idx, didx, (size_t)n_sel * sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
+  // the 16 column groups of the view, in the row order of the device block
+  const double* const src[16] = {hev->lep_px, hev->lep_py, hev->lep_pz, hev->lep_e, hev->lep_pt, hev->lep_eta,
+                                 hev->jet_px, hev->jet_py, hev->jet_pz, hev->jet_e, hev->jet_pt, hev->jet_eta,
+                                 hev->met_x, hev->met_y, hev->met, hev->mll};
+  const int rows[16] = {2, 2, 2, 2, 2, 2, 8, 8, 8, 8, 8, 8, 1, 1, 1, 1};
+  const double* dptr[16];
+  { int64_t row = 0; for (int b = 0; b < 16; b++) { dptr[b] = dcols + row * dstride; row += rows[b]; } }
+  // chunks of consecutive events; boundaries are multiples of 4 so that every chunk view keeps the 16-byte alignment
+  int nc = (int)(n / MIN_CHUNK); if (nc < 1) nc = 1; if (nc > MAX_CHUNKS) nc = MAX_CHUNKS;
+  const int64_t cs = ((n + nc - 1) / nc + 3) / 4 * 4;
+  // ---- host -> device, all chunks, on the copy-in stream (ordered after whatever the caller's stream holds) ----------
+  HEPF_CUDA_TRY(cudaEventRecord(g_pipe.start, stream));
+  HEPF_CUDA_TRY(cudaStreamWaitEvent(g_pipe.in, g_pipe.start, 0));
+  HEPF_CUDA_TRY(cudaStreamWaitEvent(g_pipe.out, g_pipe.start, 0));
+  for (int c = 0; c < nc; c++) {
+    const int64_t lo = c * cs, len = (lo + cs <= n ? cs : n - lo);
+    if (len <= 0) { nc = c; break; }
+    for (int b = 0; b < 16; b++)
+      HEPF_CUDA_TRY(cudaMemcpy2DAsync(const_cast<double*>(dptr[b]) + lo, dstride * sizeof(double), src[b] + lo,
+                                      hev->stride * sizeof(double), (size_t)len * sizeof(double), rows[b],
+                                      cudaMemcpyHostToDevice, g_pipe.in));
+    HEPF_CUDA_TRY(cudaMemcpyAsync(dflags + lo, hev->flags + lo, (size_t)len * sizeof(uint32_t), cudaMemcpyHostToDevice, g_pipe.in));
+    HEPF_CUDA_TRY(cudaEventRecord(g_pipe.arrived[c], g_pipe.in));
   }
-  if (host_out_cutflow && n_cuts > 0)
-    HEPF_CUDA_TRY(cudaMemcpyAsync(host_out_cutflow, dcutflow, (size_t)n_cuts * sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
+  // ---- per chunk: select + reconstruct on the chunk view, results device -> host on the copy-out stream --------------
+  int64_t total = 0;
+  for (int c = 0; c < nc; c++) {
+    const int64_t lo = c * cs, len = (lo + cs <= n ? cs : n - lo);
+    hepf_events_t view = *hev;
+    view.n_events = len; view.stride = dstride; view.event_base = hev->event_base + lo;
+    const double** vp[16] = {&view.lep_px, &view.lep_py, &view.lep_pz, &view.lep_e, &view.lep_pt, &view.lep_eta,
+                             &view.jet_px, &view.jet_py, &view.jet_pz, &view.jet_e, &view.jet_pt, &view.jet_eta,
+                             &view.met_x, &view.met_y, &view.met, &view.mll};
+    for (int b = 0; b < 16; b++) *vp[b] = dptr[b] + lo;
+    view.flags = dflags + lo;
+    HEPF_CUDA_TRY(cudaStreamWaitEvent(stream, g_pipe.arrived[c], 0));
+    rc = hepf_select(&view, host_cuts, n_cuts, didx + total, dcount + c, host_out_cutflow ? dcutflow + c * HEPF_MAX_CUTS : nullptr,
+                     base + L.sel_ws, up256(hepf_select_workspace_bytes(n)), stream);
+    if (rc != HEPF_OK) return rc;
+    int64_t n_sel = 0;
+    HEPF_CUDA_TRY(cudaMemcpyAsync(&n_sel, dcount + c, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
+    HEPF_CUDA_TRY(cudaStreamSynchronize(stream));     // the reconstruction takes its list length as a host value
+    if (n_sel > 0) {
+      rc = reconstruct_impl(&view, didx + total, n_sel, n_variations, seed, host_params, dbest + total, base + L.reco_ws,
+                            up256(hepf_reconstruct_workspace_bytes(n, 1)), stream, lo);
+      if (rc != HEPF_OK) return rc;
+      if (lo > 0) {
+        add_offset_kernel<<<(unsigned)((n_sel + 255) / 256), 256, 0, stream>>>(didx + total, n_sel, (uint32_t)lo);
+        count_launch();
+      }
+      HEPF_CUDA_TRY(cudaEventRecord(g_pipe.done[c], stream));
+      HEPF_CUDA_TRY(cudaStreamWaitEvent(g_pipe.out, g_pipe.done[c], 0));
+      HEPF_CUDA_TRY(cudaMemcpyAsync(host_out_best + total, dbest + total, (size_t)n_sel * sizeof(hepf_best_t),
+                                    cudaMemcpyDeviceToHost, g_pipe.out));
+      if (host_out_idx)
+        HEPF_CUDA_TRY(cudaMemcpyAsync(host_out_idx + total, didx + total, (size_t)n_sel * sizeof(uint32_t),
+                                      cudaMemcpyDeviceToHost, g_pipe.out));
+    }
+    total += n_sel;
+  }
+  *host_out_count = total;
+  if (host_out_cutflow && n_cuts > 0) {
+    int64_t cf[MAX_CHUNKS * HEPF_MAX_CUTS];
+    HEPF_CUDA_TRY(cudaMemcpyAsync(cf, dcutflow, (size_t)nc * HEPF_MAX_CUTS * sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
+    HEPF_CUDA_TRY(cudaStreamSynchronize(stream));
+    for (int k = 0; k < n_cuts; k++) { host_out_cutflow[k] = 0; for (int c = 0; c < nc; c++) host_out_cutflow[k] += cf[c * HEPF_MAX_CUTS + k]; }
+  }
+  HEPF_CUDA_TRY(cudaStreamSynchronize(g_pipe.out));
   HEPF_CUDA_TRY(cudaStreamSynchronize(stream));
   return HEPF_OK;
 }

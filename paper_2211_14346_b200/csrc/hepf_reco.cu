@@ -41,6 +41,7 @@ struct RecoCols {
   const double *lep_px, *lep_py, *lep_pz, *lep_e, *jet_px, *jet_py, *jet_pz, *jet_e, *met_x, *met_y;
   const uint32_t* flags;
   int64_t n, stride, event_base;
+  int64_t out_off;   // added to the `event` field of the records (hepf_tth_host reconstructs chunk views of one sample)
 };
 
 struct V4 { double x, y, z, e; };
@@ -666,7 +667,7 @@ reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_id
     o->nu[0] = o->nu[1] = o->nu[2] = o->nubar[0] = o->nubar[1] = o->nubar[2] = n;
     o->m_top = o->m_antitop = o->m_wplus = o->m_wminus = o->m_higgs = o->loglik = n;
     o->variation = o->jet_b = o->jet_bbar = o->jet_h1 = o->jet_h2 = o->root = -1;
-    o->status = h.status; o->event = (uint32_t)h.e;
+    o->status = h.status; o->event = (uint32_t)(h.e + ev.out_off);
     return;
   }
   const int v = (int)(w.x >> 11), a6 = (w.x >> 5) & 63, i = a6 / 6, j = a6 - 6 * i, hsel = (w.x >> 2) & 7, ksel = w.x & 3;
@@ -741,7 +742,7 @@ reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_id
   o->variation = v;
   o->jet_b = si; o->jet_bbar = sj; o->jet_h1 = sh1; o->jet_h2 = sh2;
   o->root = rank;
-  o->status = h.status | 1u; o->event = (uint32_t)h.e;
+  o->status = h.status | 1u; o->event = (uint32_t)(h.e + ev.out_off);
 }
 
 // HEPF_RECO_CFG (8, 161, 163, 164) overrides the launch shape; for tuning experiments only
@@ -806,7 +807,13 @@ extern "C" size_t hepf_reconstruct_workspace_bytes(int64_t n_idx, int32_t n_vari
 extern "C" int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
                                     uint64_t seed, const hepf_tth_params_t* host_params, hepf_best_t* out_best, void* ws,
                                     size_t ws_bytes, void* stream_) {
-  cudaStream_t stream = (cudaStream_t)stream_;
+  return hepf::reconstruct_impl(events, idx, n_idx, n_variations, seed, host_params, out_best, ws, ws_bytes,
+                                (cudaStream_t)stream_, 0);
+}
+
+int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int32_t n_variations, uint64_t seed,
+                           const hepf_tth_params_t* host_params, hepf_best_t* out_best, void* ws, size_t ws_bytes,
+                           cudaStream_t stream, int64_t event_out_offset) {
   int rc = check_events(events);
   if (rc != HEPF_OK) return rc;
   if (n_idx < 0 || n_variations < 1 || n_variations > (1 << 21)) {
@@ -825,7 +832,7 @@ extern "C" int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t*
   if (host_params) P = *host_params; else hepf_default_params(&P);
   const RecoCols cols{events->lep_px, events->lep_py, events->lep_pz, events->lep_e, events->jet_px, events->jet_py,
                       events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags,
-                      events->n_events, events->stride, events->event_base};
+                      events->n_events, events->stride, events->event_base, event_out_offset};
   uint2* winners = reinterpret_cast<uint2*>(ws);
   const int cfg = reco_tuning();
   if (n_variations <= 8 || cfg == 8) rc = launch_search_both<8, 2, 12, 10>(cols, idx, n_idx, n_variations, seed, P, winners, stream);

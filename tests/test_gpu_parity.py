@@ -421,3 +421,21 @@ def test_chi2_semilep_parity(hepf):
     assert hepf.chi2_semilep(dev, idx_t, 0).shape[0] == 0
     with pytest.raises(hepf.HepfError):
         hepf.chi2_semilep(dev, idx_t, 5, (172.5, 80.4, 0.0, 7.5))
+
+
+def test_tth_host_pipelined_chunks_equal_device_path(hepf):
+    """hepf_tth_host cuts a large sample into chunk views that are copied, selected and reconstructed in a pipeline; the
+    result must be byte-identical to the single-view device path (global-index keying, event field offsets, cutflow sums),
+    also for a host view with a stride larger than the event count and an odd size."""
+    cfg = hs.CONFIGS[1]
+    n = 300_003
+    st = cfg.events(n)
+    dev, idx_t, n_sel, idx, cf = _gpu_select(hepf, st, cfg.cuts)
+    want = _gpu_reco(hepf, dev, idx_t, n_sel, 3, 4242)
+    hidx, hbest, hcf = hepf.tth_host(st, cfg.cuts, 3, 4242)
+    assert np.array_equal(hidx, idx) and np.array_equal(hcf, cf)
+    assert hbest.tobytes() == want.tobytes()
+    wide = hs.EventStore(n, st.stride + 10, st.event_base, np.zeros((hs.NROW, st.stride + 10)), np.zeros(st.stride + 10, dtype=np.uint32))
+    wide.cols[:, :st.stride] = st.cols; wide.flags[:st.stride] = st.flags
+    hidx2, hbest2, hcf2 = hepf.tth_host(wide, cfg.cuts, 3, 4242)
+    assert np.array_equal(hidx2, idx) and np.array_equal(hcf2, cf) and hbest2.tobytes() == want.tobytes()
