@@ -6,13 +6,15 @@
 // probable solution wins; PAPER.md:145 — the measured momenta are varied V times within the resolution.  The
 // equations themselves are in DESIGN.md "Method" (the paper defers them to its ref. [27]).
 //
-// B200 mapping (v2).  The work is FP64-pipe bound (no bytes to speak of), so the design goal is: every FP64
+// B200 mapping.  The work is FP64-pipe bound (no bytes to speak of), so the design goal is: every FP64
 // instruction issued with 32 useful lanes, from a code body small enough to live in the instruction cache.
-//   reco_search_kernel   one WARP per selected event; the V variations are processed in chunks of VC.  Each chunk
-//                        runs a pipeline of short, convergent stages whose work items are spread over the lanes:
+//   reco_search_kernel   persistent warps draw groups of list entries from a global counter; one WARP reconstructs one
+//                        event at a time.  Once per event: nominal objects, conic frames (the variation-independent
+//                        part of every leg conic) and pairing constants.  The V variations are processed in chunks of VC;
+//                        each chunk runs a pipeline of short, convergent stages whose work items are spread over the lanes:
 //       A  (variation, Philox block)      -> 2 normals (in-register Philox4x32-10 + Box-Muller) -> 2 scales
 //       M  (variation, x|y)               -> MET' (slot-ordered sum, bit-identical to the definition)
-//       B  (variation, leg, b candidate)  -> leg conic (leg 2 shifted by MET') -> shared-memory table
+//       B  (variation, leg, b candidate)  -> (d, e, f) of the leg conic from its frame (leg 2 shifted by MET') -> shared memory
 //       H  (variation, candidate pair)    -> Higgs mass term
 //       C  (variation, ordered pairing)   -> resultant -> monic quartic -> Ferrari (FP32 seed for the resolvent cubic,
 //                                            FP64 Newton) -> 0/2/4 real roots PUSHED on a per-warp shared-memory stack
