@@ -398,10 +398,8 @@ def main():
                       "l2": (f"inputs ({516 * n / 1e6:.0f} MB of columns) larger than the 126 MB L2; no flush needed" if 516 * n > 126e6 else f"inputs ({516 * n / 1e6:.1f} MB) fit in L2: parity-test configuration, not a bench line"),
                       "parallelism": f"dp{world} (events sharded by global index, no collective)"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "select": select_line}
-    if not args.no_cpu_baseline and world == 1:
+    if not args.no_cpu_baseline and world == 1:      # the oracle is timed beside the GPU number on rank 0 at N = 1 only
         out["cpu_baseline"] = cpu_oracle_rate(store, idx_host, V, seed, chain=cfg.cuts)
-    elif not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_oracle_rate(store, idx_host, V, seed, target_s=8.0, chain=cfg.cuts)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
