@@ -18,7 +18,7 @@ constexpr int64_t MIN_CHUNK = 32768;      // events; smaller samples are not wor
 
 size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 
-struct ArenaLayout { size_t cols, flags, idx, count, cutflow, sel_ws, reco_ws, best, total; };
+struct ArenaLayout { size_t cols, flags, idx, count, cutflow, sel_ws[2], reco_ws[2], best, total; };
 
 ArenaLayout layout(int64_t n, int64_t stride) {
   ArenaLayout L{};
@@ -28,16 +28,18 @@ ArenaLayout layout(int64_t n, int64_t stride) {
   L.idx = off; off += up256((size_t)(n > 0 ? n : 1) * sizeof(uint32_t));
   L.count = off; off += 256;                                             // one int64 per chunk
   L.cutflow = off; off += up256((size_t)MAX_CHUNKS * HEPF_MAX_CUTS * sizeof(int64_t));
-  L.sel_ws = off; off += up256(hepf_select_workspace_bytes(n));
-  L.reco_ws = off; off += up256(hepf_reconstruct_workspace_bytes(n, 1));
+  for (int k = 0; k < 2; k++) {      // one set per compute stream (chunks alternate between two streams)
+    L.sel_ws[k] = off; off += up256(hepf_select_workspace_bytes(n));
+    L.reco_ws[k] = off; off += up256(hepf_reconstruct_workspace_bytes(n, 1));
+  }
   L.best = off; off += up256((size_t)(n > 0 ? n : 1) * sizeof(hepf_best_t));
   L.total = off;
   return L;
 }
 
 struct Pipe {                    // per host thread, created on first use
-  cudaStream_t in = nullptr, out = nullptr;
-  cudaEvent_t arrived[MAX_CHUNKS] = {}, done[MAX_CHUNKS] = {}, start = nullptr;
+  cudaStream_t in = nullptr, out = nullptr, alt = nullptr;   // alt: second compute stream (odd chunks)
+  cudaEvent_t arrived[MAX_CHUNKS] = {}, done[MAX_CHUNKS] = {}, start = nullptr, alt_done = nullptr;
   bool ok = false;
 };
 thread_local Pipe g_pipe;
@@ -46,6 +48,8 @@ int pipe_init() {
   if (g_pipe.ok) return HEPF_OK;
   HEPF_CUDA_TRY(cudaStreamCreateWithFlags(&g_pipe.in, cudaStreamNonBlocking));
   HEPF_CUDA_TRY(cudaStreamCreateWithFlags(&g_pipe.out, cudaStreamNonBlocking));
+  HEPF_CUDA_TRY(cudaStreamCreateWithFlags(&g_pipe.alt, cudaStreamNonBlocking));
+  HEPF_CUDA_TRY(cudaEventCreateWithFlags(&g_pipe.alt_done, cudaEventDisableTiming));
   HEPF_CUDA_TRY(cudaEventCreateWithFlags(&g_pipe.start, cudaEventDisableTiming));
   for (int c = 0; c < MAX_CHUNKS; c++) {
     HEPF_CUDA_TRY(cudaEventCreateWithFlags(&g_pipe.arrived[c], cudaEventDisableTiming));
@@ -106,6 +110,7 @@ extern "C" int hepf_tth_host(const hepf_events_t* hev, const hepf_cut_t* host_cu
   HEPF_CUDA_TRY(cudaEventRecord(g_pipe.start, stream));
   HEPF_CUDA_TRY(cudaStreamWaitEvent(g_pipe.in, g_pipe.start, 0));
   HEPF_CUDA_TRY(cudaStreamWaitEvent(g_pipe.out, g_pipe.start, 0));
+  HEPF_CUDA_TRY(cudaStreamWaitEvent(g_pipe.alt, g_pipe.start, 0));
   for (int c = 0; c < nc; c++) {
     const int64_t lo = c * cs, len = (lo + cs <= n ? cs : n - lo);
     if (len <= 0) { nc = c; break; }
@@ -127,22 +132,26 @@ extern "C" int hepf_tth_host(const hepf_events_t* hev, const hepf_cut_t* host_cu
                              &view.met_x, &view.met_y, &view.met, &view.mll};
     for (int b = 0; b < 16; b++) *vp[b] = dptr[b] + lo;
     view.flags = dflags + lo;
-    HEPF_CUDA_TRY(cudaStreamWaitEvent(stream, g_pipe.arrived[c], 0));
+    // chunks alternate between the caller's stream and a second compute stream, so that the persistent search kernel of
+    // chunk c + 1 fills the SMs that the tail of chunk c's leaves idle
+    const int w = c & 1;
+    cudaStream_t cs_ = w ? g_pipe.alt : stream;
+    HEPF_CUDA_TRY(cudaStreamWaitEvent(cs_, g_pipe.arrived[c], 0));
     rc = hepf_select(&view, host_cuts, n_cuts, didx + total, dcount + c, host_out_cutflow ? dcutflow + c * HEPF_MAX_CUTS : nullptr,
-                     base + L.sel_ws, up256(hepf_select_workspace_bytes(n)), stream);
+                     base + L.sel_ws[w], up256(hepf_select_workspace_bytes(n)), cs_);
     if (rc != HEPF_OK) return rc;
     int64_t n_sel = 0;
-    HEPF_CUDA_TRY(cudaMemcpyAsync(&n_sel, dcount + c, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
-    HEPF_CUDA_TRY(cudaStreamSynchronize(stream));     // the reconstruction takes its list length as a host value
+    HEPF_CUDA_TRY(cudaMemcpyAsync(&n_sel, dcount + c, sizeof(int64_t), cudaMemcpyDeviceToHost, cs_));
+    HEPF_CUDA_TRY(cudaStreamSynchronize(cs_));        // the reconstruction takes its list length as a host value
     if (n_sel > 0) {
-      rc = reconstruct_impl(&view, didx + total, n_sel, n_variations, seed, host_params, dbest + total, base + L.reco_ws,
-                            up256(hepf_reconstruct_workspace_bytes(n, 1)), stream, lo);
+      rc = reconstruct_impl(&view, didx + total, n_sel, n_variations, seed, host_params, dbest + total, base + L.reco_ws[w],
+                            up256(hepf_reconstruct_workspace_bytes(n, 1)), cs_, lo);
       if (rc != HEPF_OK) return rc;
       if (lo > 0) {
-        add_offset_kernel<<<(unsigned)((n_sel + 255) / 256), 256, 0, stream>>>(didx + total, n_sel, (uint32_t)lo);
+        add_offset_kernel<<<(unsigned)((n_sel + 255) / 256), 256, 0, cs_>>>(didx + total, n_sel, (uint32_t)lo);
         count_launch();
       }
-      HEPF_CUDA_TRY(cudaEventRecord(g_pipe.done[c], stream));
+      HEPF_CUDA_TRY(cudaEventRecord(g_pipe.done[c], cs_));
       HEPF_CUDA_TRY(cudaStreamWaitEvent(g_pipe.out, g_pipe.done[c], 0));
       HEPF_CUDA_TRY(cudaMemcpyAsync(host_out_best + total, dbest + total, (size_t)n_sel * sizeof(hepf_best_t),
                                     cudaMemcpyDeviceToHost, g_pipe.out));
@@ -153,6 +162,8 @@ extern "C" int hepf_tth_host(const hepf_events_t* hev, const hepf_cut_t* host_cu
     total += n_sel;
   }
   *host_out_count = total;
+  HEPF_CUDA_TRY(cudaEventRecord(g_pipe.alt_done, g_pipe.alt));        // the caller's stream ends after both compute streams
+  HEPF_CUDA_TRY(cudaStreamWaitEvent(stream, g_pipe.alt_done, 0));
   if (host_out_cutflow && n_cuts > 0) {
     int64_t cf[MAX_CHUNKS * HEPF_MAX_CUTS];
     HEPF_CUDA_TRY(cudaMemcpyAsync(cf, dcutflow, (size_t)nc * HEPF_MAX_CUTS * sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
