@@ -342,8 +342,10 @@ __device__ __forceinline__ void refine_xy(const Conic& A, const Conic& B, double
   if (fabs(D2) > 1e-12 * (fabs(L.q0) + fabs(q1x))) y = -D1 * rcp_fast(D2);
   else y = root_y_fallback(A, B, x);
   double mv = 0.0;
-#pragma unroll
-  for (int it = 0; it < 2; it++) newton_xy<false>(A, B, x, y, mv);
+  newton_xy<false>(A, B, x, y, mv);
+  // quadratic convergence: a first step below 1e-6 (relative) leaves an error of order 1e-12 of the step scale; the
+  // second step is taken by the lanes that moved more (a per-lane decision: the result depends on the root alone)
+  if (mv > 1e-6 * (fabs(x) + fabs(y))) newton_xy<false>(A, B, x, y, mv); else mv = 0.0;
   // a second step that still moved the point by more than 1e-10 (relative) means near-tangent conics (linear
   // convergence): keep polishing out of line, up to six more steps
   if (mv > 1e-10 * (fabs(x) + fabs(y))) { const double2 r = refine_more(A, B, x, y); x = r.x; y = r.y; }
