@@ -480,7 +480,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
     W.met[lane - 10] = __ldg((lane == 10 ? ev.met_x : ev.met_y) + h.e);
   }
   __syncwarp();
-  const int nb = h.n_b, n_pair = nb * (nb - 1) / 2, n_ord = nb * (nb - 1);
+  // the n_b = 4 instantiation only ever sees events with four candidates: a compile-time constant there
+  const int nb = (NBT == 4) ? 4 : h.n_b, n_pair = nb * (nb - 1) / 2, n_ord = nb * (nb - 1);
   if (lane < 2 * nb) {               // frames of (leg, candidate): once per event
     const int leg = lane >= nb, c = lane - leg * nb;
     const int ls = leg ? 1 - h.lp_slot : h.lp_slot, js = 2 + ((h.cand >> (4 * c)) & 15);
@@ -537,6 +538,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
     }
     __syncwarp();
     // ---- B: leg conics (leg 0: l+ with candidate c; leg 1: l- with candidate c, shifted by MET') -------------------------
+#pragma unroll 1
     for (int c0 = 0; c0 < 2 * nb; c0 += LPB) {
       const int comb = c0 + sub;
       if (vok && comb < 2 * nb) {
@@ -556,6 +558,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       }
     }
     // ---- H: Higgs term of every unordered candidate pair ---------------------------------------------------------------
+#pragma unroll 1
     for (int p0 = 0; p0 < n_pair; p0 += LPB) {
       const int p = p0 + sub;
       if (vok && p < n_pair) {
@@ -568,6 +571,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
     }
     __syncwarp();
     // ---- C: ordered pairings -> quartic -> roots pushed on the stack; D: pop 32 roots at a time ---------------------------
+#pragma unroll 1
     for (int a0 = 0; a0 < n_ord; a0 += LPB) {
       const int ap = a0 + sub;
       int mask = 0; uint32_t tag = 0;
