@@ -439,9 +439,10 @@ template <int VC, int NBT>
 struct __align__(16) WarpMem {
   static constexpr int NP = NBT * (NBT - 1) / 2;
   double def[3][2 * NBT * VC];   // (d, e, f) of the conic of (leg, candidate, variation); lanes of a pass differ in the variation
-  double fr[FRN][2 * NBT];       // per event: frame of (leg, candidate) incl. the quadratic part (a, b, c)
+  double fr[FRN - 2][2 * NBT];   // per event: frame of (leg, candidate) without (a, b): c, c1, c2, d1, d2, g1, g2, h1, ile, hml2, hmb2, bln
   double rs[10 * VC];            // reciprocal scales
-  double pc[4][NBT * (NBT - 1)];  // per event: pair constants (p2, q1, r3, 1/h4) of every ordered pairing
+  double2 pcv[NBT * (NBT - 1)][2];  // per event: pair constants (p2, q1), (r3, 1/h4) of every ordered pairing (128-bit loads)
+  double2 ab[2 * NBT];              // per event: (a, b) of the frame of (leg, candidate), read with one 128-bit load
   double ht[VC * NP];            // Higgs term of candidate pair (k, l), k < l
   double sc[VC * 10];            // scales of the ten objects
   double M[VC * 2];              // MET'
@@ -468,8 +469,9 @@ __device__ __forceinline__ void score_entry(const WarpMem<VC, NBT>& W, double x,
                                             double& best_ll, uint32_t& best_key) {
   const int vv = tag & 31, i = (tag >> 5) & 7, j = (tag >> 8) & 7, h = (tag >> 11) & 7, t = (tag >> 14) & 15, k = (tag >> 18) & 3;
   const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
-  const Conic A{W.fr[0][i], W.fr[1][i], W.fr[2][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
-  const Conic B{W.fr[0][NBT + j], W.fr[1][NBT + j], W.fr[2][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
+  const double2 abA = W.ab[i], abB = W.ab[NBT + j];
+  const Conic A{abA.x, abA.y, W.fr[0][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
+  const Conic B{abB.x, abB.y, W.fr[0][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
   double y;
   refine_xy(A, B, x, y);
   const double ll = loglik_of(x, y, W.M[vv], W.M[VC + vv], W.ht[t * VC + vv], inv_lambda);
@@ -498,9 +500,10 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
     const int ls = leg ? 1 - h.lp_slot : h.lp_slot, js = 2 + ((h.cand >> (4 * c)) & 15);
     const Frame F = make_frame(&W.obj[ls * 4], &W.obj[js * 4]);
     const int fi = leg * NBT + c;
-    W.fr[0][fi] = F.a; W.fr[1][fi] = F.b; W.fr[2][fi] = F.c; W.fr[3][fi] = F.c1; W.fr[4][fi] = F.c2;
-    W.fr[5][fi] = F.d1; W.fr[6][fi] = F.d2; W.fr[7][fi] = F.g1; W.fr[8][fi] = F.g2; W.fr[9][fi] = F.h1;
-    W.fr[10][fi] = F.ile; W.fr[11][fi] = F.hml2; W.fr[12][fi] = F.hmb2; W.fr[13][fi] = F.bln;
+    W.ab[fi] = make_double2(F.a, F.b);
+    W.fr[0][fi] = F.c; W.fr[1][fi] = F.c1; W.fr[2][fi] = F.c2;
+    W.fr[3][fi] = F.d1; W.fr[4][fi] = F.d2; W.fr[5][fi] = F.g1; W.fr[6][fi] = F.g2; W.fr[7][fi] = F.h1;
+    W.fr[8][fi] = F.ile; W.fr[9][fi] = F.hml2; W.fr[10][fi] = F.hmb2; W.fr[11][fi] = F.bln;
   }
   __syncwarp();
   const uint64_t PK = pair_k_list(nb), PL = pair_l_list(nb);
@@ -508,8 +511,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   const int dmul = nb == 4 ? 11 : (nb == 5 ? 1 : 13), dsh = nb == 4 ? 5 : (nb == 5 ? 2 : 6);
   if (lane < n_ord) {                // pair constants of every ordered pairing: once per event
     const int i = (lane * dmul) >> dsh; int j = lane - i * (nb - 1); j += (j >= i);
-    const PairConst K = pair_consts(W.fr[0][i], W.fr[1][i], W.fr[2][i], W.fr[0][NBT + j], W.fr[1][NBT + j], W.fr[2][NBT + j]);
-    W.pc[0][lane] = K.p2; W.pc[1][lane] = K.q1; W.pc[2][lane] = K.r3; W.pc[3][lane] = K.ih4;
+    const PairConst K = pair_consts(W.ab[i].x, W.ab[i].y, W.fr[0][i], W.ab[NBT + j].x, W.ab[NBT + j].y, W.fr[0][NBT + j]);
+    W.pcv[lane][0] = make_double2(K.p2, K.q1); W.pcv[lane][1] = make_double2(K.r3, K.ih4);
   }
   __syncwarp();
   const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2), inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
@@ -557,9 +560,9 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         const int ls = leg ? 1 - h.lp_slot : h.lp_slot, js = 2 + ((h.cand >> (4 * c)) & 15);
         const int fi = leg * NBT + c;
         Frame F;
-        F.a = W.fr[0][fi]; F.b = W.fr[1][fi]; F.c = W.fr[2][fi]; F.c1 = W.fr[3][fi]; F.c2 = W.fr[4][fi];
-        F.d1 = W.fr[5][fi]; F.d2 = W.fr[6][fi]; F.g1 = W.fr[7][fi]; F.g2 = W.fr[8][fi]; F.h1 = W.fr[9][fi];
-        F.ile = W.fr[10][fi]; F.hml2 = W.fr[11][fi]; F.hmb2 = W.fr[12][fi]; F.bln = W.fr[13][fi];
+        F.a = W.ab[fi].x; F.b = W.ab[fi].y; F.c = W.fr[0][fi]; F.c1 = W.fr[1][fi]; F.c2 = W.fr[2][fi];
+        F.d1 = W.fr[3][fi]; F.d2 = W.fr[4][fi]; F.g1 = W.fr[5][fi]; F.g2 = W.fr[6][fi]; F.h1 = W.fr[7][fi];
+        F.ile = W.fr[8][fi]; F.hml2 = W.fr[9][fi]; F.hmb2 = W.fr[10][fi]; F.bln = W.fr[11][fi];
         Conic q; double c0_;
         q.a = F.a; q.b = F.b; q.c = F.c;
         conic_def(F, W.sc[ls * VC + vv], W.sc[js * VC + vv], W.rs[ls * VC + vv], W.rs[js * VC + vv], hmw2, hcm, c0_, q.d, q.e, q.f);
@@ -590,9 +593,10 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       if (vok && ap < n_ord) {
         const int i = (ap * dmul) >> dsh; int j = ap - i * (nb - 1); j += (j >= i);   // i = ap / (nb - 1)
         const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
-        const Conic A{W.fr[0][i], W.fr[1][i], W.fr[2][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
-        const Conic B{W.fr[0][NBT + j], W.fr[1][NBT + j], W.fr[2][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
-        const PairConst K{W.pc[0][ap], W.pc[1][ap], W.pc[2][ap], W.pc[3][ap]};
+        const double2 abA = W.ab[i], abB = W.ab[NBT + j], k01 = W.pcv[ap][0], k23 = W.pcv[ap][1];
+        const Conic A{abA.x, abA.y, W.fr[0][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
+        const Conic B{abB.x, abB.y, W.fr[0][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
+        const PairConst K{k01.x, k01.y, k23.x, k23.y};
         double g3, g2, g1, g0;
         resultant(A, B, K, g3, g2, g1, g0);
         mask = solve_quartic(g3, g2, g1, g0, seedE, xa, xb);
