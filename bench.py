@@ -32,7 +32,7 @@ UNIT = "reconstructions/s"
 FP64_LANES_PER_SM = 64
 # Algorithmic FP64 work of one solve: the search kernel's own predicated-on thread-level FP64 instruction counts per
 # solve (idle lanes and divergence waste do not count), from the committed ncu capture of this build
-# (profiles/r01g_final.md): DADD + DMUL + DFMA lane-ops, and flop with FMA = 2.  DESIGN.md section 7.
+# (profiles/r01g_final.md, r01h_final.md): DADD + DMUL + DFMA lane-ops, and flop with FMA = 2.  DESIGN.md section 7.
 FP64_OPS_PER_SOLVE = {"dadd": 33.8, "dmul": 75.0, "dfma": 125.9}
 FP64_OPS_PER_SOLVE_NB6 = {"dadd": 26.5, "dmul": 60.7, "dfma": 101.9}   # n_b = 6 kernel (cfg3), profiles/r01g
 DRAM_BYTES_PER_LAUNCH = 276.3e6   # ncu dram__bytes_read.sum + dram__bytes_write.sum of the search kernel (same profile)
@@ -377,7 +377,7 @@ def main():
                 "peak_source": f"{sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max:.0f} MHz (DESIGN.md section 6.2)",
                 "fp64_lane_ops_per_solve": LANE_OPS_PER_SOLVE, "flop_per_solve": FLOP_PER_SOLVE,
                 "tflops_fma2": achieved, "tflops_fma2_peak": peak_tflops, "dfma_chain_measured_tflops": fma_peak,
-                "ncu_sm__pipe_fp64_cycles_active_pct": None if nb6 or args.workload != "cfg2" else 48.0,
+                "ncu_sm__pipe_fp64_cycles_active_pct": None if nb6 or args.workload != "cfg2" else 49.9,
                 "kernel_ms": ms_search, "kernel_share_of_step": ms_search / ms_per_step,
                 "other_kernels_ms": {"reco_search_other_class": float(np.mean(k_search if nb6 else k_search6)),
                                      "select_eval+scatter": float(np.mean(k_sel)), "reco_finalize": float(np.mean(k_final)),
