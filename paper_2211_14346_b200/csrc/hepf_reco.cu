@@ -475,8 +475,10 @@ __device__ __forceinline__ void score_entry(const WarpMem<VC, NBT>& W, double x,
   double y;
   refine_xy(A, B, x, y);
   const double ll = loglik_of(x, y, W.M[vv], W.M[VC + vv], W.ht[t * VC + vv], inv_lambda);
-  const uint32_t key = make_key(v0 + vv, i, j, h, k);
-  if (ll > best_ll || (ll == best_ll && key < best_key)) { best_ll = ll; best_key = key; }
+  if (ll >= best_ll) {               // the key is only needed by a candidate that can replace the incumbent (rare per lane)
+    const uint32_t key = make_key(v0 + vv, i, j, h, k);
+    if (ll > best_ll || key < best_key) { best_ll = ll; best_key = key; }
+  }
 }
 
 // One event, all variations, by one warp (see the header of this file).  Returns the winner key in every lane.
