@@ -377,7 +377,7 @@ def main():
                 "peak_source": f"{sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max:.0f} MHz (DESIGN.md section 6.2)",
                 "fp64_lane_ops_per_solve": LANE_OPS_PER_SOLVE, "flop_per_solve": FLOP_PER_SOLVE,
                 "tflops_fma2": achieved, "tflops_fma2_peak": peak_tflops, "dfma_chain_measured_tflops": fma_peak,
-                "ncu_sm__pipe_fp64_cycles_active_pct": None if nb6 or args.workload != "cfg2" else 49.9,
+                "ncu_sm__pipe_fp64_cycles_active_pct": None if nb6 or args.workload != "cfg2" else 50.0,
                 "kernel_ms": ms_search, "kernel_share_of_step": ms_search / ms_per_step,
                 "other_kernels_ms": {"reco_search_other_class": float(np.mean(k_search if nb6 else k_search6)),
                                      "select_eval+scatter": float(np.mean(k_sel)), "reco_finalize": float(np.mean(k_final)),
