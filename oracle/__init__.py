@@ -55,7 +55,7 @@ class Pairing(C.Structure):
                 ("conic1", C.c_double * 6), ("conic2", C.c_double * 6), ("x", C.c_double * 4),
                 ("kappa", C.c_double * 4), ("nterm", C.c_double * 4), ("nu", (C.c_double * 4) * 4),
                 ("nubar", (C.c_double * 4) * 4), ("hterm", C.c_double * 6), ("mbb", C.c_double * 6),
-                ("min_abs_p_rel", C.c_double)]
+                ("min_abs_p_rel", C.c_double), ("pz_terms", C.c_double * 4), ("pzbar_terms", C.c_double * 4)]
 
 
 _lib = None
@@ -78,6 +78,7 @@ def lib():
                                     C.POINTER(Params), C.POINTER(Pairing)]
         L.orc_smear.argtypes = [C.POINTER(Events), C.c_uint32, C.c_int32, C.c_uint64, C.POINTER(Params),
                                 C.c_void_p, C.c_void_p]
+        L.orc_quartic.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]
         L.orc_nu_pz.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_void_p]
         L.orc_chi2_semilep.argtypes = [C.POINTER(Events), C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_histogram.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int32, C.c_void_p]
@@ -179,6 +180,16 @@ def eval_cell(store, e: int, v: int, a: int, seed: int, params: Params | None = 
     if rc < 0:
         raise RuntimeError(f"orc_eval_cell: {rc}")
     return out
+
+
+def quartic(g):
+    """(ascending simple real roots, tangency measure) of the monic quartic x^4 + g[3] x^3 + g[2] x^2 + g[1] x + g[0]."""
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    roots, m = np.zeros(4), C.c_double()
+    n = lib().orc_quartic(g.ctypes.data, roots.ctypes.data, C.byref(m))
+    if n < 0:
+        raise RuntimeError(f"orc_quartic: {n}")
+    return roots[:n].copy(), m.value
 
 
 def smear(store, e: int, v: int, seed: int, params: Params | None = None):

@@ -76,6 +76,7 @@ typedef struct {      /* one pairing solved in isolation (worked example, brute-
   double nu[4][4], nubar[4][4];  /* px py pz E per root                                        */
   double hterm[6], mbb[6];
   double min_abs_p_rel; /* min over critical points of |P|/sum|h_i x^i| (near-tangency measure) */
+  double pz_terms[4], pzbar_terms[4]; /* per root: |c0|+|c1 x|+|c2 y| of the two p_z linear forms */
 } orc_pairing_t;
 
 void orc_default_params(orc_params_t* p);
@@ -100,6 +101,8 @@ int orc_solve_pairing(const double lp[4], const double b[4], const double lm[4],
 /* the (event, variation, pairing a) cell of orc_reconstruct_tth, re-evaluated on request */
 int orc_eval_cell(const orc_events_t* ev, uint32_t e, int32_t v, int32_t a, uint64_t seed,
                   const orc_params_t* params, orc_pairing_t* out);
+/* the root finder alone: real simple roots (ascending) of the monic quartic g0..g3 and its tangency measure */
+int orc_quartic(const double g[4], double roots[4], double* min_abs_p_rel);
 /* smeared objects of one (event, variation): scales[10], met'[2] */
 int orc_smear(const orc_events_t* ev, uint32_t e, int32_t v, uint64_t seed, const orc_params_t* params,
               double scales[10], double metp[2]);

@@ -157,6 +157,25 @@ int quartic_roots(const double g[4], double roots[4]) {
   return n;
 }
 
+// near-tangency measure (R11 iii): min over the critical points of P of |P| / sum |g_i x^i| (1 if P' has no
+// real root inside the Cauchy bound)
+double tangency_measure(const double g[4]) {
+  double m = 1.0;
+  double P1[4] = {g[1], 2.0 * g[2], 3.0 * g[3], 4.0}, P2[3] = {2.0 * g[2], 6.0 * g[3], 12.0};
+  double Rb = 1.0; for (int i = 0; i < 4; i++) Rb = std::max(Rb, 1.0 + std::fabs(g[i]));
+  double c2[2]; int n2 = 0; double disc = P2[1] * P2[1] - 4.0 * P2[2] * P2[0];
+  if (disc > 0.0) { double sq = std::sqrt(disc); c2[0] = (-P2[1] - sq) / 24.0; c2[1] = (-P2[1] + sq) / 24.0; n2 = 2; }
+  double c1[3]; int n1 = roots_between(P1, 3, c2, n2, Rb, c1);
+  double Pm[5] = {g[0], g[1], g[2], g[3], 1.0};
+  for (int i = 0; i < n1; i++) {
+    double xx = c1[i], sum = 0.0, xp = 1.0;
+    for (int j = 0; j <= 4; j++) { sum += std::fabs(Pm[j] * xp); xp *= xx; }
+    double rel = std::fabs(poly(Pm, 4, xx)) / sum;
+    if (rel < m) m = rel;
+  }
+  return m;
+}
+
 struct PairingSolution {
   int n_roots = 0;
   double x[4], y[4], kappa[4], nterm[4], sz[4], szb[4];   // sz: sum of |terms| of the p_z linear forms (R11b)
@@ -177,38 +196,15 @@ PairingSolution solve_pairing(const V4& lp, const V4& b, const V4& lm, const V4&
   for (int i = 0; i < 4; i++) { S.g[i] = h[i] / h[4]; if (!std::isfinite(S.g[i])) return S; }
   double roots[4];
   int n = quartic_roots(S.g, roots);
-  // near-tangency measure (R11 iii): min over critical points of |P| / sum |h_i x^i|
-  {
-    double P1[4] = {S.g[1], 2.0 * S.g[2], 3.0 * S.g[3], 4.0}, P2[3] = {2.0 * S.g[2], 6.0 * S.g[3], 12.0};
-    double Rb = 1.0; for (int i = 0; i < 4; i++) Rb = std::max(Rb, 1.0 + std::fabs(S.g[i]));
-    double c2[2]; int n2 = 0; double disc = P2[1] * P2[1] - 4.0 * P2[2] * P2[0];
-    if (disc > 0.0) { double sq = std::sqrt(disc); c2[0] = (-P2[1] - sq) / 24.0; c2[1] = (-P2[1] + sq) / 24.0; n2 = 2; }
-    double c1[3]; int n1 = roots_between(P1, 3, c2, n2, Rb, c1);
-    double Pm[5] = {S.g[0], S.g[1], S.g[2], S.g[3], 1.0};
-    for (int i = 0; i < n1; i++) {
-      double xx = c1[i], sum = 0.0, xp = 1.0;
-      for (int j = 0; j <= 4; j++) { sum += std::fabs(Pm[j] * xp); xp *= xx; }
-      double rel = std::fabs(poly(Pm, 4, xx)) / sum;
-      if (rel < S.min_abs_p_rel) S.min_abs_p_rel = rel;
-    }
-  }
+  S.min_abs_p_rel = tangency_measure(S.g);
   for (int r = 0; r < n; r++) {
     double x = roots[r];
     double D1 = S.R.p[0] + S.R.p[1] * x + S.R.p[2] * x * x;
     double D2 = S.R.q[0] + S.R.q[1] * x;
-    double y;
-    if (std::fabs(D2) > 1e-12 * (std::fabs(S.R.q[0]) + std::fabs(S.R.q[1] * x))) {
-      y = -D1 / D2;
-    } else {  // conics share the y-direction at this x: solve conic 1 for y, keep the y closer to conic 2
-      double qa = S.k1.c, qb = S.k1.b * x + S.k1.e, qc = S.k1.a * x * x + S.k1.d * x + S.k1.f;
-      double dd = qb * qb - 4.0 * qa * qc;
-      if (!(dd >= 0.0) || qa == 0.0) continue;
-      double sq = std::sqrt(dd), y1 = (-qb - sq) / (2.0 * qa), y2 = (-qb + sq) / (2.0 * qa);
-      auto res2 = [&](double yy) {
-        return std::fabs(S.k2.a * x * x + S.k2.b * x * yy + S.k2.c * yy * yy + S.k2.d * x + S.k2.e * yy + S.k2.f);
-      };
-      y = res2(y1) <= res2(y2) ? y1 : y2;
-    }
+    // D2(x) = 0: both conics have the same two y at this x, i.e. x is a double root of P, which the method skips
+    // (SURVEY.md 8(c) O4 "exact double roots are skipped"; R11c).  The quotient is then not finite.
+    double y = -D1 / D2;
+    if (!std::isfinite(y)) continue;
     // Two Newton steps on the pair of conics in (x, y) — the defining equations of the intersection.  The
     // quotient -D1/D2 cancels catastrophically when D2(x) is small, and north_star asks for 1e-9 (R11a).
     for (int it = 0; it < 2; it++) {
@@ -219,8 +215,10 @@ PairingSolution solve_pairing(const V4& lp, const V4& b, const V4& lm, const V4&
       double F2x = 2.0 * B.a * x + B.b * y + B.d, F2y = B.b * x + 2.0 * B.c * y + B.e;
       double det = F1x * F2y - F1y * F2x;
       double dx = (F1 * F2y - F2 * F1y) / det, dy = (F1x * F2 - F2x * F1) / det;
-      if (std::isfinite(dx) && std::isfinite(dy)) { x = x - dx; y = y - dy; }
+      x = x - dx; y = y - dy;
     }
+    // a singular Jacobian at the intersection means tangent conics, again a double root: skipped (R11c)
+    if (!std::isfinite(x) || !std::isfinite(y)) continue;
     int i = S.n_roots;
     S.x[i] = x; S.y[i] = y;
     double pz = g1.c0 + g1.c1 * x + g1.c2 * y;
@@ -367,6 +365,7 @@ void export_pairing(const PairingSolution& S, orc_pairing_t* out) {
   }
   for (int r = 0; r < S.n_roots; r++) {
     out->x[r] = S.x[r]; out->kappa[r] = S.kappa[r]; out->nterm[r] = S.nterm[r];
+    out->pz_terms[r] = S.sz[r]; out->pzbar_terms[r] = S.szb[r];
     out->nu[r][0] = S.nu[r].x; out->nu[r][1] = S.nu[r].y; out->nu[r][2] = S.nu[r].z; out->nu[r][3] = S.nu[r].e;
     out->nubar[r][0] = S.nub[r].x; out->nubar[r][1] = S.nub[r].y; out->nubar[r][2] = S.nub[r].z;
     out->nubar[r][3] = S.nub[r].e;
@@ -405,6 +404,12 @@ extern "C" int orc_solve_pairing(const double lp[4], const double b[4], const do
   }
   out->n_higgs = h;
   return 0;
+}
+
+extern "C" int orc_quartic(const double g[4], double roots[4], double* min_abs_p_rel) {
+  if (!g || !roots) return -1;
+  if (min_abs_p_rel) *min_abs_p_rel = tangency_measure(g);
+  return quartic_roots(g, roots);
 }
 
 extern "C" int orc_smear(const orc_events_t* ev, uint32_t e, int32_t v, uint64_t seed, const orc_params_t* params,

@@ -30,8 +30,6 @@
 // No tensor cores: nothing here is a contraction.
 #include <math_constants.h>
 
-#include <cstdlib>
-
 #include "hepf_common.cuh"
 
 namespace hepf {
@@ -295,16 +293,6 @@ __device__ __forceinline__ double conic_at(const Conic& k, double x, double y) {
   return fma(fma(k.a, x, fma(k.b, y, k.d)), x, fma(fma(k.c, y, k.e), y, k.f));
 }
 
-// y of a root x: y = -D1(x)/D2(x); when the conics share the y direction at x, solve conic 1 and keep the
-// y closer to conic 2 (step 3).
-__device__ __noinline__ double root_y_fallback(const Conic k1, const Conic k2, double x) {
-  const double qa = k1.c, qb = fma(k1.b, x, k1.e), qc = fma(fma(k1.a, x, k1.d), x, k1.f);
-  const double dd = fma(qb, qb, -4.0 * qa * qc);
-  if (!(dd >= 0.0) || qa == 0.0) return CUDART_NAN;
-  const double sq = sqrt(dd), y1 = (-qb - sq) / (2.0 * qa), y2 = (-qb + sq) / (2.0 * qa);
-  return fabs(conic_at(k2, x, y1)) <= fabs(conic_at(k2, x, y2)) ? y1 : y2;
-}
-
 // one Newton step on the pair of conics in (x, y); mv = |dx| + |dy| (left unchanged, and the point kept, if the
 // Jacobian is singular)
 template <bool GUARD>
@@ -338,9 +326,10 @@ __device__ __noinline__ double2 refine_more(const Conic A, const Conic B, double
 // itself (R11a).
 __device__ __forceinline__ void refine_xy(const Conic& A, const Conic& B, double& x, double& y) {
   const Lines L = lines_of(A, B);
-  const double D1 = fma(fma(L.p2, x, L.p1), x, L.p0), q1x = L.q1 * x, D2 = L.q0 + q1x;
-  if (fabs(D2) > 1e-12 * (fabs(L.q0) + fabs(q1x))) y = -D1 * rcp_fast(D2);
-  else y = root_y_fallback(A, B, x);
+  // D2(x) = 0 means the two conics share both y at this x: a double root in x, which the method skips (R11c);
+  // the quotient is then non-finite, so is the refined point, and a NaN never wins the argmax
+  const double D1 = fma(fma(L.p2, x, L.p1), x, L.p0), D2 = fma(L.q1, x, L.q0);
+  y = -D1 * rcp_fast(D2);
   double mv = 0.0;
   newton_xy<false>(A, B, x, y, mv);
   // quadratic convergence: a first step below 1e-6 (relative) leaves an error of order 1e-12 of the step scale; the
@@ -358,6 +347,98 @@ __device__ __forceinline__ double loglik_of(double x, double y, double Mx, doubl
   return ht + fma(-(ptn + ptb), inv_lambda, ln_fast(ptn * ptb));
 }
 
+
+// ---- winner polish in double-double (finalize kernel only) ---------------------------------------------------------------
+// The search compares candidates in plain FP64, which is all a ranking needs.  The reported solution, however, should
+// be the solution of the DEFINITION (the four mass constraints on the smeared FP64 four-vectors plus
+// the MET' balance) to the 1e-9 that north_star asks, also where the intersection of the two conics is ill-conditioned
+// (near-tangent conics, small n_z: an FP64 evaluation loses cond x 2^-53, R11).  So the one winner per event is
+// polished by Newton on the RAW constraints in (p_x, p_y, p_z, q_z), residuals evaluated in double-double arithmetic
+// (error-free sums and products, ~106 bits) from the exact inputs, the Jacobian in FP64: every step gains about
+// -log10(cond x 2^-53) digits, and the result is rounded once at the end.  About 1 % of the search's time in total.
+struct DD { double hi, lo; };
+__device__ __forceinline__ DD dd_fast2sum(double a, double b) { const double s = a + b; return DD{s, b - (s - a)}; }
+__device__ __forceinline__ DD dd_2sum(double a, double b) { const double s = a + b, v = s - a; return DD{s, (a - (s - v)) + (b - v)}; }
+__device__ __forceinline__ DD dd_2prod(double a, double b) { const double p = a * b; return DD{p, fma(a, b, -p)}; }
+__device__ __forceinline__ DD dd_add(DD a, DD b) {
+  DD s = dd_2sum(a.hi, b.hi); const DD t = dd_2sum(a.lo, b.lo);
+  s = dd_fast2sum(s.hi, s.lo + t.hi);
+  return dd_fast2sum(s.hi, s.lo + t.lo);
+}
+__device__ __forceinline__ DD dd_neg(DD a) { return DD{-a.hi, -a.lo}; }
+__device__ __forceinline__ DD dd_sub(DD a, DD b) { return dd_add(a, dd_neg(b)); }
+__device__ __forceinline__ DD dd_mul(DD a, DD b) { DD p = dd_2prod(a.hi, b.hi); p.lo += a.hi * b.lo + a.lo * b.hi; return dd_fast2sum(p.hi, p.lo); }
+__device__ __forceinline__ DD dd_muld(DD a, double b) { DD p = dd_2prod(a.hi, b); p.lo += a.lo * b; return dd_fast2sum(p.hi, p.lo); }
+__device__ __forceinline__ DD dd_sqrt(DD a) {
+  const double s = sqrt(a.hi);
+  const DD r = dd_sub(a, dd_2prod(s, s));
+  return dd_fast2sum(s, r.hi / (2.0 * s));
+}
+// Minkowski product of two FP64 four-vectors (x, y, z, e), exact products, double-double sums
+__device__ __forceinline__ DD dd_dot4(const V4& u, const V4& v) {
+  return dd_sub(dd_2prod(u.e, v.e), dd_add(dd_add(dd_2prod(u.x, v.x), dd_2prod(u.y, v.y)), dd_2prod(u.z, v.z)));
+}
+// residuals of one leg: (l + n)^2 - m_W^2 and (l + n + b)^2 - m_t^2 for the massless n = (p, |p|)
+__device__ __forceinline__ void dd_leg_residuals(const V4& l, const V4& b, const DD p[3], DD E, DD mw2, DD mt2, double& fw, double& ft) {
+  const DD ml2 = dd_dot4(l, l), mb2 = dd_dot4(b, b), lb = dd_dot4(l, b);
+  const DD lp = dd_sub(dd_muld(E, l.e), dd_add(dd_add(dd_muld(p[0], l.x), dd_muld(p[1], l.y)), dd_muld(p[2], l.z)));
+  const DD bp = dd_sub(dd_muld(E, b.e), dd_add(dd_add(dd_muld(p[0], b.x), dd_muld(p[1], b.y)), dd_muld(p[2], b.z)));
+  const DD w = dd_sub(dd_add(ml2, dd_add(lp, lp)), mw2);                       // m_l^2 + 2 l.n - m_W^2
+  DD t = dd_add(dd_add(ml2, mb2), dd_add(lb, lb));                            // (l + b)^2
+  t = dd_sub(dd_add(t, dd_add(dd_add(lp, lp), dd_add(bp, bp))), mt2);         // + 2 (l + b).n - m_t^2
+  fw = w.hi + w.lo; ft = t.hi + t.lo;
+}
+// Returns false (and leaves the point alone) if the iteration does not settle next to where it started.
+__device__ __noinline__ bool polish_raw(const V4 lp, const V4 bi, const V4 lm, const V4 bj, double Mx, double My, double m_top,
+                                        double m_w, double& x, double& y, double& pz, double& qx, double& qy, double& qz) {
+  const DD mw2 = dd_2prod(m_w, m_w), mt2 = dd_2prod(m_top, m_top);
+  DD u[4] = {DD{x, 0.0}, DD{y, 0.0}, DD{pz, 0.0}, DD{qz, 0.0}};
+  const double scale = fabs(x) + fabs(y) + fabs(pz) + fabs(qz);
+  double mv = CUDART_INF, total = 0.0;
+#pragma unroll 1
+  for (int it = 0; it < 6 && mv > 1e-24 * scale; it++) {
+    const DD q[3] = {dd_sub(DD{Mx, 0.0}, u[0]), dd_sub(DD{My, 0.0}, u[1]), u[3]};
+    const DD p[3] = {u[0], u[1], u[2]};
+    const DD E = dd_sqrt(dd_add(dd_add(dd_mul(p[0], p[0]), dd_mul(p[1], p[1])), dd_mul(p[2], p[2])));
+    const DD Eq = dd_sqrt(dd_add(dd_add(dd_mul(q[0], q[0]), dd_mul(q[1], q[1])), dd_mul(q[2], q[2])));
+    double A[4][5];
+    dd_leg_residuals(lp, bi, p, E, mw2, mt2, A[0][4], A[1][4]);
+    dd_leg_residuals(lm, bj, q, Eq, mw2, mt2, A[2][4], A[3][4]);
+    const double ie = 1.0 / E.hi, iq = 1.0 / Eq.hi;
+    const double ux = p[0].hi * ie, uy = p[1].hi * ie, uz = p[2].hi * ie, vx = q[0].hi * iq, vy = q[1].hi * iq, vz = q[2].hi * iq;
+    const double s1 = lp.e, s2 = lp.e + bi.e, t1 = lm.e, t2 = lm.e + bj.e;
+    A[0][0] = 2.0 * (s1 * ux - lp.x); A[0][1] = 2.0 * (s1 * uy - lp.y); A[0][2] = 2.0 * (s1 * uz - lp.z); A[0][3] = 0.0;
+    A[1][0] = 2.0 * (s2 * ux - (lp.x + bi.x)); A[1][1] = 2.0 * (s2 * uy - (lp.y + bi.y)); A[1][2] = 2.0 * (s2 * uz - (lp.z + bi.z)); A[1][3] = 0.0;
+    A[2][0] = -2.0 * (t1 * vx - lm.x); A[2][1] = -2.0 * (t1 * vy - lm.y); A[2][2] = 0.0; A[2][3] = 2.0 * (t1 * vz - lm.z);
+    A[3][0] = -2.0 * (t2 * vx - (lm.x + bj.x)); A[3][1] = -2.0 * (t2 * vy - (lm.y + bj.y)); A[3][2] = 0.0; A[3][3] = 2.0 * (t2 * vz - (lm.z + bj.z));
+    // Gaussian elimination with partial pivoting (rows swapped in place)
+    for (int c = 0; c < 4; c++) {
+      int pr = c;
+      for (int r = c + 1; r < 4; r++) if (fabs(A[r][c]) > fabs(A[pr][c])) pr = r;
+      for (int k = 0; k < 5; k++) { const double t = A[c][k]; A[c][k] = A[pr][k]; A[pr][k] = t; }
+      const double ip = 1.0 / A[c][c];
+      for (int r = c + 1; r < 4; r++) {
+        const double m = A[r][c] * ip;
+        for (int k = c; k < 5; k++) A[r][k] -= m * A[c][k];
+      }
+    }
+    double d[4];
+    for (int c = 3; c >= 0; c--) {
+      double sacc = A[c][4];
+      for (int k = c + 1; k < 4; k++) sacc -= A[c][k] * d[k];
+      d[c] = sacc / A[c][c];
+    }
+    mv = fabs(d[0]) + fabs(d[1]) + fabs(d[2]) + fabs(d[3]);
+    total += mv;
+    if (!(total <= 1e-3 * scale)) return false;     // NaN, or wandering off to another intersection
+    for (int c = 0; c < 4; c++) u[c] = dd_sub(u[c], DD{d[c], 0.0});
+  }
+  if (!(mv <= 1e-18 * scale)) return false;
+  const DD fqx = dd_sub(DD{Mx, 0.0}, u[0]), fqy = dd_sub(DD{My, 0.0}, u[1]);
+  x = u[0].hi; y = u[1].hi; pz = u[2].hi; qz = u[3].hi; qx = fqx.hi; qy = fqy.hi;
+  return true;
+}
+
 struct EventHead {   // what a warp / thread needs to know about its event
   int64_t e;         // index inside the view
   uint64_t gidx;     // global index (keys the smearing stream)
@@ -370,7 +451,8 @@ struct EventHead {   // what a warp / thread needs to know about its event
 __device__ __forceinline__ EventHead load_head(const RecoCols& ev, int64_t e) {
   EventHead h;
   h.e = e; h.gidx = (uint64_t)(ev.event_base + e);
-  const uint32_t f = __ldg(ev.flags + e);
+  const bool in_range = (uint64_t)e < (uint64_t)ev.n;       // idx[k] >= n_events: flags 0 -> not applicable, status 2 | 8
+  const uint32_t f = in_range ? __ldg(ev.flags + e) : 0u;
   const int n_lep = f & 15u;
   h.n_jet = min(8u, (f >> 8) & 15u);
   const bool q0 = (f >> 4) & 1u, q1 = (f >> 5) & 1u;
@@ -382,6 +464,7 @@ __device__ __forceinline__ EventHead load_head(const RecoCols& ev, int64_t e) {
     h.cand |= (uint32_t)s << (4 * c); h.n_b++;
   }
   if (n_tag > NBM) h.status |= 4u;
+  if (!in_range) h.status |= 8u;
   h.applicable = (n_lep == 2) && (q0 != q1) && (h.n_b >= 4);
   if (!h.applicable) h.status |= 2u;
   h.lp_slot = q0 ? 0 : 1;
@@ -520,7 +603,9 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2), inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
   const unsigned lt = (1u << lane) - 1u;
   const int seedE = seed_scale(P);
-  double best_ll = -CUDART_INF;
+  // a candidate must beat the most negative finite double: a loglik of -inf (p_T = 0) or NaN is not a solution, exactly
+  // as the definition's strict '>' against an initial -inf
+  double best_ll = -1.7976931348623157e308;
   uint32_t best_key = 0xffffffffu;
   int qn = 0;                                      // stack height (warp-uniform)
 
@@ -759,27 +844,23 @@ reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_id
   const V4 h1 = scale_v4(obj[2 + sh1], sc[2 + sh1]), h2 = scale_v4(obj[2 + sh2], sc[2 + sh2]);
   const double mbb = mass_of(h1.e + h2.e, h1.x + h2.x, h1.y + h2.y, h1.z + h2.z);
   const double t = (mbb - P.m_higgs) * inv_sh, ht = -0.5 * (t * t);
-  const double pz = fma(c2, yy, fma(c1, xx, c0));
-  const double qx = Mx - xx, qy = My - yy, qz = fma(e2, qy, fma(e1, qx, e0));
-  const double en = sqrt_fast(fma(xx, xx, fma(yy, yy, pz * pz))), eb = sqrt_fast(fma(qx, qx, fma(qy, qy, qz * qz)));
-  o->nu[0] = xx; o->nu[1] = yy; o->nu[2] = pz;
+  double pz = fma(c2, yy, fma(c1, xx, c0));
+  double qx = Mx - xx, qy = My - yy, qz = fma(e2, qy, fma(e1, qx, e0));
+  double xx_ = xx, yy_ = yy;
+  if (nr) polish_raw(lp, bi, lm, bj, Mx, My, P.m_top, P.m_w, xx_, yy_, pz, qx, qy, qz);
+  const double en = sqrt_fast(fma(xx_, xx_, fma(yy_, yy_, pz * pz))), eb = sqrt_fast(fma(qx, qx, fma(qy, qy, qz * qz)));
+  o->nu[0] = xx_; o->nu[1] = yy_; o->nu[2] = pz;
   o->nubar[0] = qx; o->nubar[1] = qy; o->nubar[2] = qz;
-  o->m_wplus = mass_of(lp.e + en, lp.x + xx, lp.y + yy, lp.z + pz);
-  o->m_top = mass_of(lp.e + en + bi.e, lp.x + xx + bi.x, lp.y + yy + bi.y, lp.z + pz + bi.z);
+  o->m_wplus = mass_of(lp.e + en, lp.x + xx_, lp.y + yy_, lp.z + pz);
+  o->m_top = mass_of(lp.e + en + bi.e, lp.x + xx_ + bi.x, lp.y + yy_ + bi.y, lp.z + pz + bi.z);
   o->m_wminus = mass_of(lm.e + eb, lm.x + qx, lm.y + qy, lm.z + qz);
   o->m_antitop = mass_of(lm.e + eb + bj.e, lm.x + qx + bj.x, lm.y + qy + bj.y, lm.z + qz + bj.z);
   o->m_higgs = mbb;
-  o->loglik = loglik_of(xx, yy, Mx, My, ht, inv_lambda);
+  o->loglik = loglik_of(xx_, yy_, Mx, My, ht, inv_lambda);
   o->variation = v;
   o->jet_b = si; o->jet_bbar = sj; o->jet_h1 = sh1; o->jet_h2 = sh2;
   o->root = rank;
   o->status = h.status | 1u; o->event = (uint32_t)(h.e + ev.out_off);
-}
-
-// HEPF_RECO_CFG (8, 161, 163, 164) overrides the launch shape; for tuning experiments only
-static int reco_tuning() {
-  static const int v = [] { const char* e = getenv("HEPF_RECO_CFG"); return e ? atoi(e) : 0; }();
-  return v;
 }
 
 template <int VC, int NBT, int RW, int MINB>
@@ -787,15 +868,17 @@ static int launch_search(const RecoCols& cols, const uint32_t* idx, int64_t n_id
                          const hepf_tth_params_t& P, uint2* winners, unsigned long long* counter, cudaStream_t stream) {
   const size_t smem = sizeof(WarpMem<VC, NBT>) * RW;
   auto kern = reco_search_kernel<VC, NBT, RW, MINB>;
-  static thread_local int blocks_per_sm = 0, sms = 0;
-  if (!blocks_per_sm) {
-    int dev = 0;
-    HEPF_CUDA_TRY(cudaGetDevice(&dev));
+  static thread_local int blocks_per_sm = 0, sms = 0, cached_dev = -1;   // per instantiation (smem is a constant of it) and device
+  int dev = 0;
+  HEPF_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev != cached_dev) {
+    blocks_per_sm = 0;
     HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     HEPF_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     HEPF_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     HEPF_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, 32 * RW, smem));
     if (blocks_per_sm < 1) { set_error("hepf_reconstruct_tth: search kernel does not fit on an SM"); return HEPF_ERR_CUDA; }
+    cached_dev = dev;
   }
   // persistent grid; groups of up to 8 list entries, fewer when the list is short
   const int64_t max_warps = (int64_t)sms * blocks_per_sm * RW;
@@ -865,14 +948,7 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, int
                       events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags,
                       events->n_events, events->stride, events->event_base, event_out_offset};
   uint2* winners = reinterpret_cast<uint2*>(ws);
-  const int cfg = reco_tuning();
-  if (n_variations <= 8 || cfg == 8) rc = launch_search_both<8, 2, 12, 10>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
-  else if (cfg == 161) rc = launch_search_both<16, 1, 20, 14>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
-  else if (cfg == 163) rc = launch_search_both<16, 2, 8, 6>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
-  else if (cfg == 165) rc = launch_search_both<16, 2, 11, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
-  else if (cfg == 166) rc = launch_search_both<16, 1, 22, 14>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
-  else if (cfg == 164) rc = launch_search_both<16, 4, 5, 3>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
-  else if (cfg == 167) rc = launch_search_both<16, 2, 10, 8>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  if (n_variations <= 8) rc = launch_search_both<8, 2, 12, 10>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   else rc = launch_search_both<16, 2, 10, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   if (rc != HEPF_OK) return rc;
   const int64_t fblocks = (n_idx + 127) / 128;

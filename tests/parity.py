@@ -1,9 +1,28 @@
-"""GPU-vs-oracle comparison of hepf_best_t records with the conditioning-aware rules of DESIGN.md R11.
+"""GPU-vs-oracle comparison of hepf_best_t records (R11).
 
-north_star: chosen indices bit-exact "except where the oracle's top two likelihoods differ by < 1e-9 relative";
-masses and momenta within 1e-9 relative in FP64.  The solve is ill-conditioned near tangent conics, so the
-per-event tolerance is max(1e-9, 64 kappa) with kappa = eps sum|h_i x^i| / |x P'(x)| reported by the oracle, and an
-index mismatch is excused only in the classes below; everything else fails.
+BASELINE.json:north_star: chosen indices bit-exact "except where the oracle's top two likelihoods differ by < 1e-9
+relative"; masses and momenta within 1e-9 relative in FP64.
+
+Tier 1 is exactly that: same indices, every value within 1e-9 of the ORACLE.  The solve is ill-conditioned near tangent
+conics and for small n_z, and the oracle is itself an FP64 evaluation: on a fraction of a percent of the events it is
+more than 1e-9 away from the exact solution of its own definition (measured in tests/test_referee.py).  A record that
+misses tier 1 is therefore taken to a REFEREE (tests/referee_q128.c: the definition of DESIGN.md section 2 in IEEE
+binary128, independent of both sides) and passes only if the GPU's record is within 1e-9 of the EXACT solution — i.e. the
+oracle is the far side.  No tolerance is widened by a model (the kappa / p_z tiers of round 1 are gone).
+
+Index mismatches are judged on exact likelihoods of the two picks:
+  tie_exact            the exact logliks of the two picks agree to 1e-9 relative (north_star's near-tie rule, on exact values)
+  oracle_misranked     the GPU's pick is exactly better; the oracle has the root but its FP64 loglik is off
+  oracle_missed_root   the GPU's pick is exactly better and is a root pair so close to tangency that the oracle's own FP64
+                       quartic (its coefficient error measured against binary128) cannot resolve it
+  gpu_missed_tangent   the oracle's pick is exactly better but sits at such a tangency (same measured criterion)
+  within_fp64_noise    the oracle's pick is exactly better by less than 4x the oracle's own measured FP64 loglik error on
+                       the two picks: an FP64 ranking cannot resolve the order
+  tangent_both         same indices, but the winning root is at a tangency that the FP64 quartic cannot resolve (measured
+                       criterion as above): in exact arithmetic the pair is double or absent, nothing beyond the indices is defined
+  tangent_gpu_only     the GPU's pick is such a root and the oracle's is a different candidate that is not exactly better by
+                       more than 1e-6
+Everything else fails.  Excused classes are counted, printed and capped.
 """
 from __future__ import annotations
 
@@ -13,9 +32,12 @@ from collections import Counter
 import numpy as np
 
 import oracle
+import referee
 
 IDX_KEYS = ("variation", "jet_b", "jet_bbar", "jet_h1", "jet_h2", "root")
-TANGENT = 1e-11     # |P| / sum|h_i x^i| at a critical point below this = near-tangent conics (class iii)
+TOL = 1e-9                      # north_star
+EPS = 2.0 ** -53
+MASS_KEYS = ("m_top", "m_antitop", "m_wplus", "m_wminus")
 
 
 def _cands(flags: int):
@@ -24,6 +46,7 @@ def _cands(flags: int):
 
 
 def _cell_of(store, rec):
+    """(pairing a = i n_b + j, Higgs pair index h) of a record's jet slots."""
     c = _cands(int(store.flags[rec["event"]]))
     nb = len(c)
     i, j = c.index(int(rec["jet_b"])), c.index(int(rec["jet_bbar"]))
@@ -38,102 +61,153 @@ def _close(a, b, tol, scale=None):
     return bool(np.all(np.abs(a - b) <= tol * s))
 
 
-def compare(store, gpu, orc, aux, n_variations, seed, params=None, m_top=172.5, m_w=80.4):
+def _tier1(g, o) -> bool:
+    pscale = max(np.abs(o["nu"]).max(), np.abs(o["nubar"]).max())
+    return (_close(g["nu"], o["nu"], TOL, pscale) and _close(g["nubar"], o["nubar"], TOL, pscale)
+            and _close(g["loglik"], o["loglik"], TOL, max(1.0, abs(o["loglik"])))
+            and all(_close(g[f], o[f], TOL, o[f]) for f in MASS_KEYS + ("m_higgs",)))
+
+
+def _mass_tol(cl, r, m):
+    """Masses are recomputed from the FP64 output four-vectors (DESIGN.md section 2 step 6): m^2 = E^2 - |p|^2 cancels, so the
+    rounding of the outputs (2^-53 each) is amplified by about (E / m)^2.  1e-9 unless that factor is larger."""
+    e_sys = cl.nu[r][3] + cl.nubar[r][3] + cl.lp[3] + cl.lm[3] + cl.b[3] + cl.bbar[3]
+    return max(TOL, 32.0 * EPS * (e_sys / m) ** 2)
+
+
+class _Exact:
+    """What the referee says about one record of either side: the exact root it sits on, its distance, the exact loglik."""
+
+    def __init__(self, store, rec, seed, rp, m_top, m_w):
+        self.ok = False
+        if not (int(rec["status"]) & 1):
+            self.ll = -math.inf; self.cl = None; self.r = None; self.err = math.inf
+            return
+        self.a, self.h = _cell_of(store, rec)
+        self.cl = referee.cell(store, int(rec["event"]), int(rec["variation"]), self.a, seed, rp)
+        self.r = referee.nearest_root(self.cl, rec["nu"][:2])
+        if self.r is None:
+            self.ll = -math.inf; self.err = math.inf
+            return
+        self.err = referee.record_error(self.cl, self.r, rec)
+        self.ll = self.cl.hterm[self.h] + self.cl.nterm[self.r]
+        cl, r = self.cl, self.r
+        self.values_ok = (self.err <= TOL
+                          and abs(rec["loglik"] - self.ll) <= TOL * max(1.0, abs(self.ll))
+                          and abs(rec["m_higgs"] - cl.mbb[self.h]) <= TOL * max(1.0, cl.mbb[self.h])
+                          and all(abs(rec[f] - m) <= _mass_tol(cl, r, m) * m
+                                  for f, m in zip(MASS_KEYS, (m_top, m_top, m_w, m_w))))
+        self.ok = True
+
+    def fragile(self, store, rec, seed, op) -> bool:
+        """Is this root one of a pair that the oracle's own FP64 quartic cannot resolve?  |P| at the critical point next to
+        the root, relative to sum|g_i x^i| (exact), against the measured coefficient error of the oracle's FP64 quartic there."""
+        cl = self.cl
+        if cl is None or cl.n_crit == 0:
+            return False
+        P = oracle.eval_cell(store, int(rec["event"]), int(rec["variation"]), self.a, seed, op)
+        x = float(rec["nu"][0])
+        k = int(np.argmin([abs(cl.crit_x[c] - x) for c in range(cl.n_crit)]))
+        c = cl.crit_x[k]
+        g_ex = list(cl.g) + [1.0]
+        g_or = list(P.g) + [1.0]
+        denom = sum(abs(g_ex[i] * c ** i) for i in range(5))
+        noise = sum(abs((g_or[i] - g_ex[i]) * c ** i) for i in range(5)) / denom
+        return cl.crit_rel[k] <= 8.0 * max(noise, 64 * EPS)
+
+
+def compare(store, gpu, orc, aux, n_variations, seed, params=None, m_top=None, m_w=None):
     """Returns (Counter of classes, list of failure strings)."""
     cls, fails = Counter(), []
+    rp = referee.params(params)
+    m_top = rp.m_top if m_top is None else m_top
+    m_w = rp.m_w if m_w is None else m_w
     for k in range(len(orc)):
         g, o, ax = gpu[k], orc[k], aux[k]
         e = int(o["event"])
         if int(g["event"]) != e:
             fails.append(f"k={k}: event {g['event']} != {e}"); continue
-        if (int(g["status"]) & 6) != (int(o["status"]) & 6):
+        if (int(g["status"]) & 14) != (int(o["status"]) & 6):
             fails.append(f"e={e}: applicability/truncation bits {g['status']} != {o['status']}"); continue
         gs, os_ = int(g["status"]) & 1, int(o["status"]) & 1
-        kap = float(ax["kappa"]) if np.isfinite(ax["kappa"]) else 0.0
-        tiers = [("match", 1e-9), ("match_kappa_tol", max(1e-9, 64 * kap))]
-        if os_:   # R11b: first-order error propagation through the p_z linear forms (large when n_z is small)
-            pn = max(np.abs(o["nu"]).max(), np.abs(o["nubar"]).max())
-            amp = max(1.0, float(ax["pz_terms"]) / pn, float(ax["pzbar_terms"]) / pn)
-            tiers.append(("match_pz_tol", tiers[1][1] * amp))
-        tol = tiers[-1][1]
         if not gs and not os_:
             ok = all(np.isnan(g[f]).all() for f in ("nu", "nubar", "loglik", "m_top")) and all(g[f] == -1 for f in IDX_KEYS)
             cls["both_unsolved"] += 1
             if not ok:
                 fails.append(f"e={e}: unsolved record is not NaN/-1")
             continue
-        if gs and os_ and all(int(g[f]) == int(o[f]) for f in IDX_KEYS):
-            pscale = max(np.abs(o["nu"]).max(), np.abs(o["nubar"]).max())
-
-            def values_ok(t):
-                return (_close(g["nu"], o["nu"], t, pscale) and _close(g["nubar"], o["nubar"], t, pscale)
-                        and _close(g["loglik"], o["loglik"], t, max(1.0, abs(o["loglik"])))
-                        and all(_close(g[f], o[f], t, o[f]) for f in ("m_top", "m_antitop", "m_wplus", "m_wminus", "m_higgs")))
-            tier = next((name for name, t in tiers if values_ok(t)), None)
-            ok = tier is not None
-            # closure of the GPU record itself: the imposed masses come back
-            ok_closure = all(abs(g[f] - m) <= 10 * tol * m for f, m in (("m_top", m_top), ("m_antitop", m_top),
-                                                                        ("m_wplus", m_w), ("m_wminus", m_w)))
-            if not ok:
-                # R11 (iii'): the winning root is one of a near-double pair (conics tangent to rounding): x is only
-                # defined to sqrt(eps), y and p_z to less; indices agree, x must agree to 1e-5, the rest is not compared
-                Pw = oracle.eval_cell(store, e, int(o["variation"]), int(ax["pairing"]), seed, params)
-                if Pw.min_abs_p_rel < TANGENT and abs(g["nu"][0] - o["nu"][0]) <= 1e-5 * max(1.0, abs(o["nu"][0])):
-                    cls["tangent_same_indices"] += 1
-                    continue
-            cls[tier or "values_differ"] += 1
-            if not ok:
-                fails.append(f"e={e}: same indices, values differ beyond tol={tol:.2e} "
-                             f"(nu {g['nu']} vs {o['nu']}, ll {g['loglik']!r} vs {o['loglik']!r})")
-            elif not ok_closure:
-                fails.append(f"e={e}: closure violated m_t={g['m_top']} m_W={g['m_wplus']}")
+        same = bool(gs and os_ and all(int(g[f]) == int(o[f]) for f in IDX_KEYS))
+        if same and _tier1(g, o):
+            cls["match"] += 1
             continue
-        # ---- index or status mismatch: classify -------------------------------------------------------------------
-        why = None
-        best_o = float(o["loglik"]) if os_ else -math.inf
-        if gs:
-            a_g, h_g = _cell_of(store, g)
-            P = oracle.eval_cell(store, e, int(g["variation"]), a_g, seed, params)
-            near = None
-            for r in range(P.n_roots):
-                if abs(P.x[r] - g["nu"][0]) <= max(1e-7, 1e3 * P.kappa[r]) * max(1.0, abs(P.x[r])):
-                    near = r
-            if near is not None:
-                ll = P.hterm[h_g] + P.nterm[near]
-                if os_ and abs(ll - best_o) <= 1e-9 * max(1.0, abs(best_o)):
-                    why = "tie_equivalent_candidate"           # (i)/(ii): same likelihood up to 1e-9
-                elif os_ and abs(best_o - float(ax["loglik2"])) <= 1e-9 * max(1.0, abs(best_o)):
-                    why = "tie_top_two"
-                elif os_ and ll > best_o:
-                    why = None                                 # oracle itself prefers it?  impossible -> fail
+        # ---- tier 1 missed: the referee decides -----------------------------------------------------------------------
+        G = _Exact(store, g, seed, rp, m_top, m_w)
+        O = _Exact(store, o, seed, rp, m_top, m_w)
+        if gs and not (G.ok and G.values_ok) and G.cl is not None and G.fragile(store, g, seed, params):
+            # the GPU's winner sits at a tangency that no FP64 evaluation resolves: in exact arithmetic the pair is a double
+            # root or absent, x is defined to sqrt(eps), y and p_z to less.  Nothing can be compared beyond the indices.
+            if same:
+                cls["tangent_both"] += 1
+            elif os_ and O.ok and O.ll > float(g["loglik"]) + 1e-6 and not O.fragile(store, o, seed, params):
+                fails.append(f"e={e}: GPU picked an unresolvable tangent root over the oracle's well-defined, better winner "
+                             f"(gpu ll={g['loglik']!r}, oracle exact ll={O.ll!r})")
             else:
-                if P.min_abs_p_rel < TANGENT:                  # (iii): GPU resolved a tangency the bisection skipped
-                    closure = all(abs(g[f] - m) <= 1e-6 * m for f, m in (("m_top", m_top), ("m_antitop", m_top),
-                                                                         ("m_wplus", m_w), ("m_wminus", m_w)))
-                    if closure:
-                        why = "tangent_root_gpu_only"
-        if why is None and os_:
-            # did the GPU miss the oracle's winning root because it sits at a near-tangency?
-            a_o, _ = int(ax["pairing"]), int(ax["higgs_pair"])
-            P = oracle.eval_cell(store, e, int(o["variation"]), a_o, seed, params)
-            if P.min_abs_p_rel < TANGENT or kap > 1e-9:
-                why = "tangent_root_oracle_only"
+                cls["tangent_gpu_only"] += 1
+            continue
+        if gs and not (G.ok and G.values_ok):
+            fails.append(f"e={e}: GPU record is not within 1e-9 of an exact solution (err={G.err:.2e}, oracle err={O.err:.2e}, "
+                         f"nu {g['nu']} ll {g['loglik']!r} exact ll {G.ll!r})")
+            continue
+        if same and G.r == O.r:
+            cls["oracle_far"] += 1            # same exact root, the GPU is within 1e-9 of it, the oracle is not
+            continue
+        # ---- different picks (or the two sides sit on different exact roots of one cell) -------------------------------
+        tie = gs and os_ and abs(G.ll - O.ll) <= TOL * max(1.0, abs(O.ll))
+        why = None
+        if tie:
+            why = "tie_exact"
+        elif G.ll > O.ll:
+            # the GPU's pick is exactly better: does the oracle have that root at all?
+            P = oracle.eval_cell(store, e, int(g["variation"]), G.a, seed, params)
+            near = [r for r in range(P.n_roots) if abs(P.x[r] - g["nu"][0]) <= 1e-6 * max(1.0, abs(g["nu"][0]))]
+            if near:
+                why = "oracle_misranked"
+            elif G.fragile(store, g, seed, params):
+                why = "oracle_missed_root"
+        else:
+            if O.cl is not None and O.fragile(store, o, seed, params):
+                why = "gpu_missed_tangent"
+            elif gs and os_ and O.r is not None:
+                # the oracle's own FP64 error on the two picks (its loglik of its winner, and of the GPU's pick) against exact
+                P = oracle.eval_cell(store, e, int(g["variation"]), G.a, seed, params)
+                near = [r for r in range(P.n_roots) if abs(P.x[r] - g["nu"][0]) <= 1e-6 * max(1.0, abs(g["nu"][0]))]
+                err_pick = abs(P.hterm[G.h] + P.nterm[near[0]] - G.ll) if near else 0.0
+                err_win = abs(float(o["loglik"]) - O.ll)
+                if O.ll - G.ll <= 4.0 * max(err_pick, err_win):
+                    why = "within_fp64_noise"
         if why is None:
             fails.append(f"e={e}: UNEXCUSED mismatch gpu(status={g['status']}, v={g['variation']}, b={g['jet_b']}, "
-                         f"bbar={g['jet_bbar']}, root={g['root']}, ll={g['loglik']!r}) vs oracle(status={o['status']}, "
+                         f"bbar={g['jet_bbar']}, root={g['root']}, ll={g['loglik']!r}, exact ll={G.ll!r}) vs oracle(status={o['status']}, "
                          f"v={o['variation']}, b={o['jet_b']}, bbar={o['jet_bbar']}, root={o['root']}, ll={o['loglik']!r}, "
-                         f"ll2={ax['loglik2']!r}, kappa={kap:.2e})")
+                         f"exact ll={O.ll!r}, ll2={ax['loglik2']!r})")
         else:
             cls[why] += 1
     return cls, fails
 
 
-def assert_parity(store, gpu, orc, aux, n_variations, seed, params=None, max_excused_frac=2e-3, label=""):
+EXCUSED = ("tie_exact", "oracle_misranked", "oracle_missed_root", "gpu_missed_tangent", "within_fp64_noise", "tangent_both",
+           "tangent_gpu_only")
+
+
+def assert_parity(store, gpu, orc, aux, n_variations, seed, params=None, max_excused_frac=2e-3, max_oracle_far_frac=5e-3,
+                  label=""):
     cls, fails = compare(store, gpu, orc, aux, n_variations, seed, params)
     n = len(orc)
-    exact = cls["match"] + cls["match_kappa_tol"] + cls["match_pz_tol"] + cls["both_unsolved"] + cls["values_differ"]
-    excused = n - exact - len(fails)
-    print(f"[parity {label}] n={n} classes={dict(cls)} failures={len(fails)}")
+    excused = sum(cls[c] for c in EXCUSED)
+    solved = max(1, n - cls["both_unsolved"])
+    print(f"[parity {label}] n={n} classes={dict(cls)} failures={len(fails)} "
+          f"tier1={cls['match'] / solved:.5f} oracle_far={cls['oracle_far'] / solved:.5f} excused={excused / solved:.5f}")
     assert not fails, "\n".join(fails[:10])
     assert excused <= max(2, max_excused_frac * n), (excused, n, dict(cls))
+    assert cls["oracle_far"] <= max(2, max_oracle_far_frac * n), (cls["oracle_far"], n)
     return cls

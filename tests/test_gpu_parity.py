@@ -282,7 +282,7 @@ def test_cfg3_full_size_sampled_parity(hepf):
         assert np.median(err) < 1e-13 and np.quantile(err, 0.99) < 1e-9
     sample = np.arange(0, n, 100)           # ~4 600 events, 3.6e7 oracle solves
     want, aux = oracle.reconstruct_tth(st, idx[sample], cfg.n_variations, cfg.reco_seed, n_threads=16)
-    assert_parity(st, got[sample], want, aux, cfg.n_variations, cfg.reco_seed, max_excused_frac=0.03, label="cfg3-sampled")
+    assert_parity(st, got[sample], want, aux, cfg.n_variations, cfg.reco_seed, label="cfg3-sampled")
 
 
 def test_cfg4_full_size_select_exact_and_survivor_parity(hepf):
@@ -300,7 +300,19 @@ def test_cfg4_full_size_select_exact_and_survivor_parity(hepf):
     assert np.array_equal(got["event"], idx)
     sample = np.arange(0, n, 20)            # ~48 700 survivors, 9.4e6 oracle solves
     want, aux = oracle.reconstruct_tth(st, idx[sample], cfg.n_variations, cfg.reco_seed, n_threads=16)
-    assert_parity(st, got[sample], want, aux, cfg.n_variations, cfg.reco_seed, max_excused_frac=0.01, label="cfg4-sampled")
+    assert_parity(st, got[sample], want, aux, cfg.n_variations, cfg.reco_seed, label="cfg4-sampled")
+
+
+def test_soak_other_seed_all_selected_events(hepf):
+    """A wider net than the fixed-seed configs: every selected event of 400 000 cfg2-like events under another generator seed
+    and another reconstruction seed, V = 8 (1.5e7 oracle solves).  Same gate as everywhere: tier 1 = 1e-9 against the oracle,
+    otherwise the referee must find the GPU within 1e-9 of the exact solution; excused index classes capped at 2e-3."""
+    st = hs.generate(400_000, 20261104, with_truth=False)
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, hs.CHAIN_BASE)
+    got = _gpu_reco(hepf, dev, idx_t, n, 8, 0xABCDEF)
+    want, aux = oracle.reconstruct_tth(st, idx, 8, 0xABCDEF, n_threads=16)
+    cls = assert_parity(st, got, want, aux, 8, 0xABCDEF, max_oracle_far_frac=5e-3, label="soak")
+    assert cls["match"] > 0.99 * (n - cls["both_unsolved"])
 
 
 def test_cfg5_full_stream_sampled_windows(hepf):
