@@ -35,7 +35,8 @@
 namespace hepf {
 
 constexpr int NBM = HEPF_MAX_B;   // candidate slots in the tables
-constexpr int QCAP = 160;         // root stack: <= 31 left over + 32 lanes x 4 new roots
+constexpr int QCAP = 160;          // root stack: <= 31 left over + 4 new roots per lane of a C2 pass (the pass is cut short if it would not fit)
+constexpr int SCAP = 64;          // solve queue: <= 31 left over + 32 new quartics
 
 struct RecoCols {
   const double *lep_px, *lep_py, *lep_pz, *lep_e, *jet_px, *jet_py, *jet_pz, *jet_e, *met_x, *met_y;
@@ -257,13 +258,36 @@ __device__ __noinline__ Biquad biquadratic_roots(double p, double r, double aq) 
   return b;
 }
 
-// Real roots of x^4 + g3 x^3 + g2 x^2 + g1 x + g0 by Ferrari's closed form; the polish happens later, on the pair of
-// conics.  Roots come out as pair A (xa[0], xa[1]) and pair B (xb[0], xb[1]).  Returns bit 0 = pair A real, bit 1 = B.
-__device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, double g0, int seedE, double (&xa)[2], double (&xb)[2]) {
-  const double aq = 0.25 * g3, aq2 = aq * aq;
-  const double p = fma(-6.0, aq2, g2);
-  const double q = fma(aq, fma(8.0, aq2, -2.0 * g2), g1);
-  const double r = fma(aq2, fma(-3.0, aq2, g2), fma(-aq, g1, g0));
+// x^4 + g3 x^3 + g2 x^2 + g1 x + g0 with x = t - aq: the depressed quartic t^4 + p t^2 + q t + r
+__device__ __forceinline__ void depress(double g3, double g2, double g1, double g0, double& aq, double& p, double& q, double& r) {
+  aq = 0.25 * g3;
+  const double aq2 = aq * aq;
+  p = fma(-6.0, aq2, g2);
+  q = fma(aq, fma(8.0, aq2, -2.0 * g2), g1);
+  r = fma(aq2, fma(-3.0, aq2, g2), fma(-aq, g1, g0));
+}
+
+// Does t^4 + p t^2 + q t + r CERTAINLY have no real root?  Its discriminant, written so that it costs a dozen operations,
+//   Delta = 16 r (4 r - p^2)^2 + q^2 (144 p r - 4 p^3 - 27 q^2),
+// is positive for 0 or 4 real roots and then (p > 0 or 4 r > p^2) means 0.  About 60 % of the solves have no root (wrong
+// pairings mostly): they stop here, and only the others are queued for the closed form (stage C2), which then runs with
+// full warps.  "Certainly": Delta must exceed the rounding of its own evaluation a thousandfold; everything else — small
+// or negative Delta, NaN, overflow of an absurdly scaled quartic — goes on to the solver, whose answer is the one that
+// counts.  The result of the search therefore does not depend on this test, only its speed does.
+__device__ __forceinline__ bool certainly_no_real_root(double p, double q, double r) {
+  const double p2 = p * p, q2 = q * q, w = fma(4.0, r, -p2);
+  const double t1 = (16.0 * r) * (w * w);
+  const double u1 = (144.0 * p) * r, u2 = (4.0 * p) * p2, u3 = 27.0 * q2;
+  const double u = (u1 - u2) - u3;
+  const double delta = fma(q2, u, t1);
+  const double mag = fma(q2, (fabs(u1) + fabs(u2)) + u3, fabs(t1));
+  return delta > 1e-12 * mag && (p > 0.0 || w > 1e-12 * p2);
+}
+
+// Real roots of the depressed quartic by Ferrari's closed form, shifted back to x = t - aq; the polish happens later, on
+// the pair of conics.  Roots come out as pair A (xa[0], xa[1]) and pair B (xb[0], xb[1]).  Returns bit 0 = pair A real,
+// bit 1 = B.
+__device__ __forceinline__ int ferrari(double p, double q, double r, double aq, int seedE, double (&xa)[2], double (&xb)[2]) {
   const double c1 = fma(0.25 * p, p, -r), c0 = -0.125 * q * q, tp = 2.0 * p;
   double m = resolvent_seed(p, q, r, seedE), step = 0.0;
 #pragma unroll
@@ -287,6 +311,11 @@ __device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, do
     xa[0] = b.x[0]; xa[1] = b.x[1]; xb[0] = b.x[2]; xb[1] = b.x[3]; mask = b.mask;
   }
   return mask;
+}
+__device__ __forceinline__ int solve_quartic(double g3, double g2, double g1, double g0, int seedE, double (&xa)[2], double (&xb)[2]) {
+  double aq, p, q, r;
+  depress(g3, g2, g1, g0, aq, p, q, r);
+  return ferrari(p, q, r, aq, seedE, xa, xb);
 }
 
 __device__ __forceinline__ double conic_at(const Conic& k, double x, double y) {
@@ -523,27 +552,27 @@ struct __align__(16) WarpMem {
   static constexpr int NP = NBT * (NBT - 1) / 2;
   double def[3][2 * NBT * VC];   // (d, e, f) of the conic of (leg, candidate, variation); lanes of a pass differ in the variation
   double fr[FRN - 2][2 * NBT];   // per event: frame of (leg, candidate) without (a, b): c, c1, c2, d1, d2, g1, g2, h1, ile, hml2, hmb2, bln
-  double rs[10 * VC];            // reciprocal scales
   double2 pcv[NBT * (NBT - 1)][2];  // per event: pair constants (p2, q1), (r3, 1/h4) of every ordered pairing (128-bit loads)
   double2 ab[2 * NBT];              // per event: (a, b) of the frame of (leg, candidate), read with one 128-bit load
   double ht[VC * NP];            // Higgs term of candidate pair (k, l), k < l
-  double sc[VC * 10];            // scales of the ten objects
   double M[VC * 2];              // MET'
   double obj[10 * 4];            // nominal (px, py, pz, E)
   double ks[10];                 // kappa * sigma
   double met[2];
-  // root stack.  n_b = 4: (bits of x, tag) in one 16-byte entry -> one STS.128 / LDS.128 per root (1 % faster there);
-  // n_b > 4: separate arrays (the packed form measured 7 % slower in that instantiation)
-  ulonglong2 q[NBT == 4 ? QCAP : 1];
-  double qx[NBT == 4 ? 1 : QCAP];
-  uint32_t qtag[NBT == 4 ? 1 : QCAP];
+  // solve queue (stage C1 -> C2): depressed quartics that may have real roots, (p, q), (r, aq) and the (variation, i, j) tag
+  double2 s_pq[SCAP], s_ra[SCAP];
+  uint32_t s_tag[SCAP];
+  // root stack (stage C2 -> D): (bits of x, tag) in one 16-byte entry, one STS.128 / LDS.128 per root.
+  // The scales of the ten objects (stages A, M, B, H) live in the same bytes: both queues are empty while a chunk's
+  // tables are built, and the scales are dead once they are.
+  union { ulonglong2 q[QCAP]; double sc_[VC * 10]; };
+  static_assert(sizeof(ulonglong2) * QCAP >= sizeof(double) * VC * 10, "the scales must fit in the root stack's bytes");
+  __device__ __forceinline__ double* sc() { return sc_; }
   __device__ __forceinline__ void push(int at, double x, uint32_t tag) {
-    if (NBT == 4) q[at] = make_ulonglong2((unsigned long long)__double_as_longlong(x), tag);
-    else { qx[at] = x; qtag[at] = tag; }
+    q[at] = make_ulonglong2((unsigned long long)__double_as_longlong(x), tag);
   }
   __device__ __forceinline__ void pop(int at, double& x, uint32_t& tag) const {
-    if (NBT == 4) { const ulonglong2 en = q[at]; x = __longlong_as_double((long long)en.x); tag = (uint32_t)en.y; }
-    else { x = qx[at]; tag = qtag[at]; }
+    const ulonglong2 en = q[at]; x = __longlong_as_double((long long)en.x); tag = (uint32_t)en.y;
   }
 };
 
@@ -607,7 +636,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   // as the definition's strict '>' against an initial -inf
   double best_ll = -1.7976931348623157e308;
   uint32_t best_key = 0xffffffffu;
-  int qn = 0;                                      // stack height (warp-uniform)
+  int qn = 0, sn = 0;                              // heights of the root stack and of the solve queue (warp-uniform)
 
 #pragma unroll 1
   for (int v0 = 0; v0 < V; v0 += VC) {
@@ -621,8 +650,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         philox4x32_10((uint32_t)h.gidx, (uint32_t)(h.gidx >> 32), (uint32_t)(v0 + vv), 0x54544800u + blk, k0, k1, x);
         double ze, zo; block_normals(x, ze, zo);
         const double s0 = scale_of(W.ks[2 * blk], ze, P.s_min), s1 = scale_of(W.ks[2 * blk + 1], zo, P.s_min);
-        W.sc[(2 * blk) * VC + vv] = s0; W.sc[(2 * blk + 1) * VC + vv] = s1;
-        W.rs[(2 * blk) * VC + vv] = rcp_fast(s0); W.rs[(2 * blk + 1) * VC + vv] = rcp_fast(s1);
+        W.sc()[(2 * blk) * VC + vv] = s0; W.sc()[(2 * blk + 1) * VC + vv] = s1;
       }
     }
     __syncwarp();
@@ -633,7 +661,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       if (vok && comp < 2) {
         double acc = 0.0;
         for (int t = 0; t < 2 + h.n_jet; t++)
-          acc = __dadd_rn(acc, __dmul_rn(__dadd_rn(W.sc[t * VC + vv], -1.0), W.obj[t * 4 + comp]));
+          acc = __dadd_rn(acc, __dmul_rn(__dadd_rn(W.sc()[t * VC + vv], -1.0), W.obj[t * 4 + comp]));
         W.M[comp * VC + vv] = __dadd_rn(W.met[comp], -acc);
       }
     }
@@ -652,7 +680,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         F.ile = W.fr[8][fi]; F.hml2 = W.fr[9][fi]; F.hmb2 = W.fr[10][fi]; F.bln = W.fr[11][fi];
         Conic q; double c0_;
         q.a = F.a; q.b = F.b; q.c = F.c;
-        conic_def(F, W.sc[ls * VC + vv], W.sc[js * VC + vv], W.rs[ls * VC + vv], W.rs[js * VC + vv], hmw2, hcm, c0_, q.d, q.e, q.f);
+        const double sl = W.sc()[ls * VC + vv], sb = W.sc()[js * VC + vv];
+        conic_def(F, sl, sb, rcp_fast(sl), rcp_fast(sb), hmw2, hcm, c0_, q.d, q.e, q.f);
         if (leg) q = shift_conic(q, W.M[vv], W.M[VC + vv]);
         const int at = (leg * NBT + c) * VC + vv;
         W.def[0][at] = q.d; W.def[1][at] = q.e; W.def[2][at] = q.f;
@@ -665,60 +694,85 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       if (vok && p < n_pair) {
         const int kk = (int)(PK >> (4 * p)) & 15, ll = (int)(PL >> (4 * p)) & 15;
         const int j1 = 2 + ((h.cand >> (4 * kk)) & 15), j2 = 2 + ((h.cand >> (4 * ll)) & 15);
-        const V4 b1 = scale_v4(&W.obj[j1 * 4], W.sc[j1 * VC + vv]), b2 = scale_v4(&W.obj[j2 * 4], W.sc[j2 * VC + vv]);
+        const V4 b1 = scale_v4(&W.obj[j1 * 4], W.sc()[j1 * VC + vv]), b2 = scale_v4(&W.obj[j2 * 4], W.sc()[j2 * VC + vv]);
         const double t = (mass_of(b1.e + b2.e, b1.x + b2.x, b1.y + b2.y, b1.z + b2.z) - P.m_higgs) * inv_sh;
         W.ht[pair_index<NBT>(kk, ll) * VC + vv] = -0.5 * (t * t);
       }
     }
     __syncwarp();
-    // ---- C: ordered pairings -> quartic -> roots pushed on the stack; D: pop 32 roots at a time ---------------------------
+    // ---- C1: ordered pairings -> resultant -> depressed quartic -> "may have real roots?" -> solve queue
+    //      C2: pop 32 queued quartics -> Ferrari -> 0/2/4 real roots pushed on the root stack
+    //      D : pop 32 roots -> refine on the conics, score
+    // One more trip of the loop (last) drains what is left of both queues with partial warps: the tables of this chunk
+    // are about to be overwritten.
 #pragma unroll 1
-    for (int a0 = 0; a0 < n_ord; a0 += LPB) {
-      const int ap = a0 + sub;
-      int mask = 0; uint32_t tag = 0;
-      double xa[2], xb[2];
-      if (vok && ap < n_ord) {
-        const int i = (ap * dmul) >> dsh; int j = ap - i * (nb - 1); j += (j >= i);   // i = ap / (nb - 1)
-        const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
-        const double2 abA = W.ab[i], abB = W.ab[NBT + j], k01 = W.pcv[ap][0], k23 = W.pcv[ap][1];
-        const Conic A{abA.x, abA.y, W.fr[0][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
-        const Conic B{abB.x, abB.y, W.fr[0][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
-        const PairConst K{k01.x, k01.y, k23.x, k23.y};
-        double g3, g2, g1, g0;
-        resultant(A, B, K, g3, g2, g1, g0);
-        mask = solve_quartic(g3, g2, g1, g0, seedE, xa, xb);
-        if (mask) {
-          double ht; int hh, kk, ll;
-          best_higgs<NBT, VC>(&W.ht[vv], nb, i, j, ht, hh, kk, ll);
-          tag = (uint32_t)vv | (i << 5) | (j << 8) | (hh << 11) | (pair_index<NBT>(kk, ll) << 14);
+    for (int a0 = 0;; a0 += LPB) {
+      const bool last = a0 >= n_ord;
+      if (!last) {
+        const int ap = a0 + sub;
+        bool keep = false;
+        double qp = 0.0, qq = 0.0, qr = 0.0, qaq = 0.0; uint32_t stag = 0;
+        if (vok && ap < n_ord) {
+          const int i = (ap * dmul) >> dsh; int j = ap - i * (nb - 1); j += (j >= i);   // i = ap / (nb - 1)
+          const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
+          const double2 abA = W.ab[i], abB = W.ab[NBT + j], k01 = W.pcv[ap][0], k23 = W.pcv[ap][1];
+          const Conic A{abA.x, abA.y, W.fr[0][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
+          const Conic B{abB.x, abB.y, W.fr[0][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
+          const PairConst K{k01.x, k01.y, k23.x, k23.y};
+          double g3, g2, g1, g0;
+          resultant(A, B, K, g3, g2, g1, g0);
+          depress(g3, g2, g1, g0, qaq, qp, qq, qr);
+          keep = !certainly_no_real_root(qp, qq, qr);
+          stag = (uint32_t)vv | (i << 5) | (j << 8);
         }
-      }
-      // push: Ferrari slots are numbered over the real pairs in the order A+, A-, B+, B-
-      const unsigned bA = __ballot_sync(0xffffffffu, mask & 1), bB = __ballot_sync(0xffffffffu, mask & 2);
-      int at = qn + 2 * (__popc(bA & lt) + __popc(bB & lt));
-      if (mask & 1) {
-        W.push(at, xa[0], tag); W.push(at + 1, xa[1], tag | (1u << 18)); at += 2;
-      }
-      if (mask & 2) {
-        const uint32_t s0 = (mask & 1) ? 2u : 0u;
-        W.push(at, xb[0], tag | (s0 << 18)); W.push(at + 1, xb[1], tag | ((s0 + 1u) << 18));
-      }
-      qn += 2 * (__popc(bA) + __popc(bB));
-      __syncwarp();
-      while (qn >= 32) {
-        qn -= 32;
-        double ex; uint32_t et; W.pop(qn + lane, ex, et);
-        score_entry<VC, NBT>(W, ex, et, v0, inv_lambda, best_ll, best_key);
+        const unsigned bk = __ballot_sync(0xffffffffu, keep);
+        if (keep) {
+          const int at = sn + __popc(bk & lt);
+          W.s_pq[at] = make_double2(qp, qq); W.s_ra[at] = make_double2(qr, qaq); W.s_tag[at] = stag;
+        }
+        sn += __popc(bk);
         __syncwarp();
       }
-    }
-    // the tables are about to be overwritten: score what is left (partial warp)
-    if (qn > 0) {
-      if (lane < qn) {
-        double ex; uint32_t et; W.pop(lane, ex, et);
-        score_entry<VC, NBT>(W, ex, et, v0, inv_lambda, best_ll, best_key);
+      while (sn >= 32 || (last && (sn | qn) != 0)) {
+        const int take = min(min(32, sn), (QCAP - qn) >> 2);   // every lane may push four roots
+        if (take > 0) {                                        // (warp-uniform; 0 only while draining the root stack at the end)
+          sn -= take;
+          int mask = 0; uint32_t tag = 0;
+          double xa[2], xb[2];
+          if (lane < take) {
+            const double2 pq = W.s_pq[sn + lane], ra = W.s_ra[sn + lane];
+            const uint32_t st = W.s_tag[sn + lane];
+            mask = ferrari(pq.x, pq.y, ra.x, ra.y, seedE, xa, xb);
+            if (mask) {
+              double ht; int hh, kk, ll;
+              best_higgs<NBT, VC>(&W.ht[st & 31], nb, (st >> 5) & 7, (st >> 8) & 7, ht, hh, kk, ll);
+              tag = st | (hh << 11) | (pair_index<NBT>(kk, ll) << 14);
+            }
+          }
+          // push: Ferrari slots are numbered over the real pairs in the order A+, A-, B+, B-
+          const unsigned bA = __ballot_sync(0xffffffffu, mask & 1), bB = __ballot_sync(0xffffffffu, mask & 2);
+          int at = qn + 2 * (__popc(bA & lt) + __popc(bB & lt));
+          if (mask & 1) {
+            W.push(at, xa[0], tag); W.push(at + 1, xa[1], tag | (1u << 18)); at += 2;
+          }
+          if (mask & 2) {
+            const uint32_t s0 = (mask & 1) ? 2u : 0u;
+            W.push(at, xb[0], tag | (s0 << 18)); W.push(at + 1, xb[1], tag | ((s0 + 1u) << 18));
+          }
+          qn += 2 * (__popc(bA) + __popc(bB));
+          __syncwarp();
+        }
+        while (qn >= 32 || (last && sn == 0 && qn > 0)) {
+          const int tk = min(32, qn);
+          qn -= tk;
+          if (lane < tk) {
+            double ex; uint32_t et; W.pop(qn + lane, ex, et);
+            score_entry<VC, NBT>(W, ex, et, v0, inv_lambda, best_ll, best_key);
+          }
+          __syncwarp();
+        }
       }
-      qn = 0;
+      if (last) break;
     }
     __syncwarp();
   }
@@ -894,16 +948,16 @@ static int launch_search(const RecoCols& cols, const uint32_t* idx, int64_t n_id
 }
 
 // both candidate-count classes: n_b = 4 (tables for 4 candidates, more warps per SM) and n_b = 5, 6
-template <int VC, int RW, int MINB4, int MINB6>
+template <int VC4, int VC6, int RW, int MINB4, int MINB6>
 static int launch_search_both(const RecoCols& cols, const uint32_t* idx, int64_t n_idx, int V, uint64_t seed,
                               const hepf_tth_params_t& P, uint2* winners, cudaStream_t stream) {
   unsigned long long* counters = reinterpret_cast<unsigned long long*>(winners + n_idx);   // two group counters
   HEPF_CUDA_TRY(cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), stream));
   timing_mark(T_RECO0, stream);
-  int rc = launch_search<VC, 4, RW, MINB4>(cols, idx, n_idx, V, seed, P, winners, counters, stream);
+  int rc = launch_search<VC4, 4, RW, MINB4>(cols, idx, n_idx, V, seed, P, winners, counters, stream);
   timing_mark(T_RECO1, stream);
   if (rc != HEPF_OK) return rc;
-  rc = launch_search<VC, 6, RW, MINB6>(cols, idx, n_idx, V, seed, P, winners, counters + 1, stream);
+  rc = launch_search<VC6, 6, RW, MINB6>(cols, idx, n_idx, V, seed, P, winners, counters + 1, stream);
   timing_mark(T_RECO2, stream);
   return rc;
 }
@@ -948,8 +1002,8 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, int
                       events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags,
                       events->n_events, events->stride, events->event_base, event_out_offset};
   uint2* winners = reinterpret_cast<uint2*>(ws);
-  if (n_variations <= 8) rc = launch_search_both<8, 2, 12, 10>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
-  else rc = launch_search_both<16, 2, 10, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 12, 10>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  else rc = launch_search_both<16, 16, 2, 10, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
   if (rc != HEPF_OK) return rc;
   const int64_t fblocks = (n_idx + 127) / 128;
   reco_finalize_kernel<<<(unsigned)fblocks, 128, 0, stream>>>(cols, idx, n_idx, (uint32_t)seed, (uint32_t)(seed >> 32), P,
