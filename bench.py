@@ -2,16 +2,21 @@
 """bench.py — smeared ttH reconstructions/s on BASELINE.json configs[1] (1e6 events, 4 b-jets, V = 64, FP64).
 
 A step is one pass of the whole hot path over the batch: hepf_select (cut chain + compaction) followed by
-hepf_reconstruct_tth (Philox/Box-Muller smearing, dilepton solve, score, argmax) for every surviving event.
-`value` counts event x variation x pairing solves per second with the inputs resident in HBM; `e2e` is the same
-metric through hepf_tth_host (host buffers in, results out, copies inside the timed region).
+hepf_reconstruct_tth_n (Philox/Box-Muller smearing, dilepton solve, score, argmax; the list length stays on the device)
+for every surviving event.  `value` counts event x variation x pairing solves per second with the inputs resident in
+HBM; `e2e` is the same metric through hepf_tth_host (host buffers in, results out, copies inside the timed region).
+The default run also times the other configs of BASELINE.json (cfg3, cfg4, cfg5) and reports them under `configs`.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg1|cfg2|cfg3|cfg4]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg1|cfg2|cfg3|cfg4|cfg5|chi2]
 Under torchrun every rank runs its own shard (events keyed by global index, no data-path collective): weak scaling.
+Everything printed is measured in this run, except the per-solve FP64 instruction counts and the DRAM traffic of the
+search kernels, which only ncu can count: they are read from profiles/r02_fp64_ops.json and used only if that file's hash
+of the kernel sources matches the tree (otherwise the fields say so and the fraction falls back to the frozen round-1 count).
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -28,14 +33,30 @@ import hepf_synth as hs  # noqa: E402
 
 METRIC = "smeared ttH reconstructions/sec (event x assignment x variation)"
 UNIT = "reconstructions/s"
-# FP64 roof of one B200 from the guide's unit counts: 148 SMs x 64 FP64 FMA lanes/clk x 2 flop x clocks.max.sm
+# FP64 roof of one B200 from the guide's unit counts: 148 SMs x 64 FP64 lanes/clk x clocks.max.sm
 FP64_LANES_PER_SM = 64
-# Algorithmic FP64 work of one solve: the search kernel's own predicated-on thread-level FP64 instruction counts per
-# solve (idle lanes and divergence waste do not count), from the committed ncu capture of this build
-# (profiles/r01g_final.md, r01h_final.md): DADD + DMUL + DFMA lane-ops, and flop with FMA = 2.  DESIGN.md section 7.
-FP64_OPS_PER_SOLVE = {"dadd": 33.8, "dmul": 75.0, "dfma": 125.9}
-FP64_OPS_PER_SOLVE_NB6 = {"dadd": 26.5, "dmul": 60.7, "dfma": 101.9}   # n_b = 6 kernel (cfg3), profiles/r01g
-DRAM_BYTES_PER_LAUNCH = 276.3e6   # ncu dram__bytes_read.sum + dram__bytes_write.sum of the search kernel (same profile)
+OPS_FILE = os.path.join(ROOT, "profiles", "r02_fp64_ops.json")
+KERNEL_SOURCES = ("paper_2211_14346_b200/csrc/hepf_reco.cu", "paper_2211_14346_b200/csrc/hepf_common.cuh")
+
+
+def kernel_source_hash() -> str:
+    h = hashlib.sha256()
+    for rel in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, rel), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
+def load_profiled_ops() -> dict:
+    """ncu-counted FP64 thread instructions per solve of the search kernels (profiles/r02_fp64_ops.json).  `current` is True
+    only if the file was written for exactly these kernel sources."""
+    try:
+        d = json.load(open(OPS_FILE))
+    except (OSError, ValueError):
+        return {"current": False, "kernels": {}, "algorithmic_fp64_ops_per_solve": {}, "file": None}
+    d["current"] = d.get("source_sha256") == kernel_source_hash()
+    d["file"] = os.path.relpath(OPS_FILE, ROOT)
+    return d
 
 
 def chain_bytes_per_event(chain) -> int:
@@ -51,6 +72,36 @@ def chain_bytes_per_event(chain) -> int:
     return 4 + sum(size[c] for c in need)
 
 
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p)).get("hbm_gbs", 6650.0)), "MEASURED_PEAKS.json hbm_gbs (copy, read+write)"
+    return 6650.0, "fallback 6650 GB/s (B200_PROFILING.md)"
+
+
+def time_philox(hepf, n, steps, warmup):
+    import torch
+    out = torch.empty(n, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        hepf.philox_normal(hs.PHILOX_CFG5["seed"], 0, n, out=out, stream=stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        hepf.philox_normal(hs.PHILOX_CFG5["seed"], 0, n, out=out, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    del out
+    ms = e0.elapsed_time(e1) / steps
+    hbm, src = hbm_peak()
+    gbs = 8.0 * n / (ms * 1e-3) / 1e9
+    return {"ms_per_step": ms, "value": n / (ms * 1e-3), "unit": "normals/s",
+            "workload": f"cfg5: {n} normals, seed 7, counter 0",
+            "roofline": {"bound": "hbm", "kernel": "philox_normal_kernel<true>", "achieved": gbs, "peak": hbm, "unit": "GB/s",
+                         "frac": gbs / hbm, "traffic": None, "algorithmic_bytes": 8.0 * n, "kernel_ms": ms, "peak_source": src}}
+
+
 def run_philox(args):
     """--workload cfg5: standalone hepf_philox_normal stream (BASELINE.json configs[4]), normals/s and GB/s written."""
     import torch
@@ -58,29 +109,13 @@ def run_philox(args):
     hepf.load()
     torch.cuda.set_device(0)
     n = args.events or hs.PHILOX_CFG5["n"]
-    out = torch.empty(n, dtype=torch.float64, device="cuda")
-    stream = torch.cuda.current_stream()
-    for _ in range(max(3, args.warmup)):
-        hepf.philox_normal(hs.PHILOX_CFG5["seed"], 0, n, out=out, stream=stream)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(args.steps):
-        hepf.philox_normal(hs.PHILOX_CFG5["seed"], 0, n, out=out, stream=stream)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / args.steps
-    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
-    hbm = float(peaks.get("hbm_gbs", 6650.0))
-    gbs = 8.0 * n / (ms * 1e-3) / 1e9
-    print(json.dumps({"metric": "standard-normal FP64 draws/sec (Philox4x32-10 + Box-Muller)", "value": n / (ms * 1e-3),
-                      "unit": "normals/s", "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms,
+    W = max(3, args.warmup)
+    r = time_philox(hepf, n, args.steps, W)
+    print(json.dumps({"metric": "standard-normal FP64 draws/sec (Philox4x32-10 + Box-Muller)", "value": r["value"],
+                      "unit": "normals/s", "n_gpus": 1, "steps": args.steps, "warmup": W, "ms_per_step": r["ms_per_step"],
                       "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                      "config": {"workload": f"cfg5: {n} normals, seed 7, counter 0", "l2": "34 GB written per step, far larger than L2"},
-                      "gpu_launches": args.steps,
-                      "roofline": {"bound": "hbm", "kernel": "philox_normal_kernel<true>", "achieved": gbs, "peak": hbm,
-                                   "unit": "GB/s", "frac": gbs / hbm, "traffic": None,
-                                   "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy, read+write)" if peaks else "fallback 6650"}}))
+                      "config": {"workload": r["workload"], "l2": "34 GB written per step, far larger than L2"},
+                      "gpu_launches": args.steps, "roofline": r["roofline"]}))
 
 
 def run_chi2(args):
@@ -108,8 +143,7 @@ def run_chi2(args):
     f = st.flags[:n].astype(np.int64); nj = np.minimum((f >> 8) & 15, 8)
     # algorithmic bytes: idx 4 + flags 4 + lepton 32 + MET 16 + 32 per jet that is a candidate (<= 4 tagged + <= 4 untagged) + 80 out
     by = float((4 + 4 + 32 + 16 + 80) * n + 32 * nj.sum())
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    hbm = float(json.load(open(peaks_path)).get("hbm_gbs", 6650.0)) if os.path.exists(peaks_path) else 6650.0
+    hbm, src = hbm_peak()
     gbs = by / (ms * 1e-3) / 1e9
     print(json.dumps({"metric": "chi2-reconstructed semileptonic ttbar events/sec", "value": n / (ms * 1e-3), "unit": "events/s",
                       "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": True,
@@ -118,7 +152,7 @@ def run_chi2(args):
                                  "l2": f"{by / 1e6:.0f} MB touched per step, larger than L2"},
                       "gpu_launches": args.steps,
                       "roofline": {"bound": "hbm", "kernel": "chi2_semilep_kernel", "achieved": gbs, "peak": hbm, "unit": "GB/s",
-                                   "frac": gbs / hbm, "traffic": None, "algorithmic_bytes": by}}))
+                                   "frac": gbs / hbm, "traffic": None, "algorithmic_bytes": by, "peak_source": src}}))
 
 
 def solves_of(store, idx, n_variations: int) -> int:
@@ -173,24 +207,21 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def cpu_oracle_rate(store, idx, n_variations, seed, target_s=15.0, chain=hs.CHAIN_BASE):
-    """Time the oracle, as it stands, on a bounded sample of the same workload on the host cores."""
+def cpu_oracle_rate(store, idx, n_variations, seed, n_threads, target_s=10.0):
+    """Time the oracle (a non-optimised checker: nested bisection, everything re-enumerated per root), as it stands, on a
+    bounded sample of the same workload on the host cores.  A reported baseline; no speed-up claim may be derived from it."""
     import oracle
-    cores = os.cpu_count() or 1
-    probe = idx[:2048]
-    t0 = time.perf_counter(); oracle.reconstruct_tth(store, probe, n_variations, seed, n_threads=cores)
+    probe = idx[:256 * n_threads]
+    t0 = time.perf_counter(); oracle.reconstruct_tth(store, probe, n_variations, seed, n_threads=n_threads)
     dt = max(time.perf_counter() - t0, 1e-3)
-    m = int(min(len(idx), max(2048, 2048 * target_s / dt)))
+    m = int(min(len(idx), max(len(probe), len(probe) * target_s / dt)))
     sample = idx[:m]
-    t0 = time.perf_counter()
-    oracle.select(store, chain)                    # the oracle's selection of the whole batch is part of a step
-    t_sel = time.perf_counter() - t0
-    t0 = time.perf_counter(); oracle.reconstruct_tth(store, sample, n_variations, seed, n_threads=cores)
+    t0 = time.perf_counter(); oracle.reconstruct_tth(store, sample, n_variations, seed, n_threads=n_threads)
     dt = time.perf_counter() - t0
     n_solves = solves_of(store, sample, n_variations)
-    return {"value": n_solves / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"first {m} selected events of the workload ({n_solves} solves, {dt:.1f} s wall, OpenMP over events; "
-                      f"oracle select of all {store.n_events} events took {t_sel:.2f} s, not included)"}
+    return {"value": n_solves / dt, "unit": UNIT, "cores": n_threads, "kind": "oracle",
+            "note": "the oracle is a non-optimised checker (nested bisection, every Higgs pair re-enumerated per root): a reported baseline, no speed-up claim may be derived from it",
+            "sample": f"first {m} selected events of the workload ({n_solves} solves, {dt:.1f} s wall, {n_threads} OpenMP thread(s) over events)"}
 
 
 def run_reference(args, cfg, name):
@@ -219,9 +250,113 @@ def run_reference(args, cfg, name):
                       "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / max(1, args.steps),
                       "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                       "config": {"workload": cfg.name, "n_variations": cfg.n_variations, "sample": sample_txt},
-                      "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample_txt},
+                      "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample_txt,
+                                       "note": "non-optimised checker: a reported baseline, no speed-up claim may be derived from it"},
                       "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
                       "gpu_launches": 0}))
+
+
+class TthRun:
+    """select -> reconstruct on one resident store, device-timed."""
+
+    def __init__(self, hepf, binding, cfg, n_ev, first_event, V, params):
+        import torch
+        self.hepf, self.binding, self.cfg, self.V, self.params = hepf, binding, cfg, V, params
+        self.store = cfg.events(n_ev, first_event=first_event)
+        self.dev = hepf.DeviceEvents.from_host(self.store)
+        n = self.n = self.store.n_events
+        L = hepf.load()
+        self.stream = torch.cuda.current_stream()
+        self.out_idx = torch.empty(max(n, 1), dtype=torch.int32, device="cuda")
+        self.out_count = torch.zeros(1, dtype=torch.int64, device="cuda")
+        self.out_cf = torch.zeros(32, dtype=torch.int64, device="cuda")
+        self.ws = torch.empty(int(L.hepf_select_workspace_bytes(n)) + 256, dtype=torch.uint8, device="cuda")
+        self.out_best = torch.empty((max(n, 1), 128), dtype=torch.uint8, device="cuda")
+        self.reco_ws = torch.empty(int(L.hepf_reconstruct_workspace_bytes(n, V)) + 256, dtype=torch.uint8, device="cuda")
+
+    def step(self):
+        """One pass of the hot path; nothing comes back to the host between the two calls."""
+        h = self.hepf
+        h.select(self.dev, self.cfg.cuts, out_idx=self.out_idx, out_count=self.out_count, out_cutflow=self.out_cf, ws=self.ws,
+                 stream=self.stream)
+        h.reconstruct_tth_n(self.dev, self.out_idx, self.out_count, self.n, self.V, self.cfg.reco_seed, self.params,
+                            out_best=self.out_best, ws=self.reco_ws, stream=self.stream)
+
+    def measure(self, steps, warmup, barrier=None):
+        import torch
+        b = self.binding
+        for _ in range(warmup):
+            self.step()
+        torch.cuda.synchronize()
+        self.n_sel = int(self.out_count.item())
+        self.idx_host = self.out_idx[:self.n_sel].cpu().numpy().view(np.uint32)
+        self.n_solves = solves_of(self.store, self.idx_host, self.V)
+        if barrier:
+            barrier()
+        torch.cuda.synchronize()
+        self.hepf.launch_count(reset=True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b.timing_enable(True)
+        k = {"search4": [], "search6": [], "finalize": [], "select": [], "select_eval": []}
+        e0.record(self.stream)
+        for _ in range(steps):
+            self.step()
+            # device time of each kernel of this step, from events the library records on the stream around its launches
+            k["search4"].append(b.timing_ms(3, 4)); k["search6"].append(b.timing_ms(4, 5)); k["finalize"].append(b.timing_ms(5, 6))
+            k["select"].append(b.timing_ms(0, 2)); k["select_eval"].append(b.timing_ms(0, 1))
+        e1.record(self.stream)
+        torch.cuda.synchronize()
+        b.timing_enable(False)
+        self.launches = int(self.hepf.launch_count())
+        self.ms_total = e0.elapsed_time(e1)
+        self.kernel_ms = {name: float(np.mean(v)) for name, v in k.items()}
+        return self.ms_total / steps
+
+    def rooflines(self, ms_per_step, sm_max_mhz, sms, prof):
+        """FP64 lane-op roofline of the dominant search kernel + HBM roofline of select_eval."""
+        km = self.kernel_ms
+        nb6 = km["search6"] > km["search4"]
+        name = "reco_search_kernel<16,6>" if nb6 else ("reco_search_kernel<16,4>" if self.V > 8 else "reco_search_kernel<8,4>")
+        ms_search = km["search6"] if nb6 else km["search4"]
+        lane_peak = sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6
+        entry = prof["kernels"].get(name) if prof.get("current") else None
+        alg = prof.get("algorithmic_fp64_ops_per_solve", {}).get("nb6" if nb6 else "nb4")
+        roof = {"bound": "alu", "kernel": name, "unit": "T FP64 lane-op/s", "peak": lane_peak / 1e12,
+                "peak_source": f"{sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max_mhz:.0f} MHz (DESIGN.md section 7)",
+                "kernel_ms": ms_search, "kernel_share_of_step": ms_search / ms_per_step, "solves_per_launch": self.n_solves,
+                "other_kernels_ms": {"reco_search_other_class": km["search4"] if nb6 else km["search6"],
+                                     "select_eval+scatter": km["select"], "reco_finalize": km["finalize"]}}
+        if entry:     # the kernel's own executed (predicated-on) FP64 thread instructions, counted by ncu on exactly these sources
+            ops = entry["dadd"] + entry["dmul"] + entry["dfma"]
+            rate = ops * self.n_solves / (ms_search * 1e-3)
+            roof.update({"achieved": rate / 1e12, "frac": rate / lane_peak, "fp64_lane_ops_per_solve": ops,
+                         "tflops_fma2": (ops + entry["dfma"]) * self.n_solves / (ms_search * 1e-3) / 1e12,
+                         "ops_source": f"{prof['file']} ({entry.get('profile')}; kernel sources hash matches this tree)",
+                         "traffic": entry.get("dram_bytes_per_launch") if entry.get("workload") == self.cfg.name.split(":")[0] else None,
+                         "ncu_sm__pipe_fp64_cycles_active_pct": entry.get("ncu_sm__pipe_fp64_cycles_active_pct")})
+        else:
+            roof.update({"achieved": None, "frac": None, "traffic": None,
+                         "ops_source": "no ncu count for these kernel sources (profiles/r02_fp64_ops.json absent or stale)"})
+        if alg:       # the method's FP64 work, frozen (DESIGN.md section 7): does not shrink when the kernel does
+            rate = alg * self.n_solves / (ms_search * 1e-3)
+            roof.update({"algorithmic_fp64_ops_per_solve": alg, "algorithmic_achieved": rate / 1e12, "algorithmic_frac": rate / lane_peak})
+            if roof["frac"] is None:
+                roof.update({"achieved": rate / 1e12, "frac": rate / lane_peak,
+                             "ops_source": roof["ops_source"] + "; frac uses the frozen algorithmic count"})
+        hbm, src = hbm_peak()
+        sel_bytes = chain_bytes_per_event(self.cfg.cuts) * self.n + 4 * self.n_sel
+        sel_ms = km["select_eval"]
+        select = {"kernel": "select_eval_kernel", "events_per_s": self.n / (sel_ms * 1e-3), "bound": "hbm",
+                  "achieved": sel_bytes / (sel_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s", "peak_source": src,
+                  "frac": sel_bytes / (sel_ms * 1e-3) / 1e9 / hbm, "algorithmic_bytes": sel_bytes, "kernel_ms": sel_ms,
+                  "eval+scatter_ms": km["select"]}
+        return roof, select
+
+    def free(self):
+        import torch
+        for a in ("dev", "out_idx", "out_best", "ws", "reco_ws", "store"):
+            setattr(self, a, None)
+        torch.cuda.empty_cache()
 
 
 def main():
@@ -233,6 +368,7 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "chi2"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra-configs", action="store_true", help="skip the cfg3 / cfg4 / cfg5 lines of the default run")
     ap.add_argument("--variations", type=int, default=0, help="override the workload's V (SURVEY 8(f) NEXT-1: 128 = ttH_scinp, 1024 = ttH_sci)")
     ap.add_argument("--sigma-scale", type=float, default=None, help="0 = no smearing, the paper's ttH_as variant")
     args = ap.parse_args()
@@ -259,68 +395,24 @@ def main():
     hepf.load()
     W = max(3, args.warmup)
     n_ev = args.events or cfg.n_events
-    # weak scaling: rank r owns global events [r n, (r+1) n); the Philox keys use the global index
-    store = cfg.events(n_ev, first_event=rank * n_ev)
-    dev = hepf.DeviceEvents.from_host(store)
-    n, V, seed = store.n_events, (args.variations or cfg.n_variations), cfg.reco_seed
+    V = args.variations or cfg.n_variations
     params = hepf.default_params(sigma_scale=args.sigma_scale) if args.sigma_scale is not None else None
-    stream = torch.cuda.current_stream()
-    out_idx = torch.empty(max(n, 1), dtype=torch.int32, device="cuda")
-    out_count = torch.zeros(1, dtype=torch.int64, device="cuda")
-    out_cf = torch.zeros(32, dtype=torch.int64, device="cuda")
-    ws = torch.empty(int(hepf.load().hepf_select_workspace_bytes(n)) + 256, dtype=torch.uint8, device="cuda")
-    out_best = torch.empty((max(n, 1), 128), dtype=torch.uint8, device="cuda")
-    reco_ws = torch.empty(int(hepf.load().hepf_reconstruct_workspace_bytes(n, V)) + 256, dtype=torch.uint8, device="cuda")
-    count_host = torch.zeros(1, dtype=torch.int64).pin_memory()
-
-    def step(ev_mid=None):
-        hepf.select(dev, cfg.cuts, out_idx=out_idx, out_count=out_count, out_cutflow=out_cf, ws=ws, stream=stream)
-        count_host.copy_(out_count, non_blocking=True)
-        stream.synchronize()                       # hepf_reconstruct_tth takes n_idx as a host value
-        n_sel = int(count_host[0])
-        if ev_mid is not None:
-            ev_mid[0].record(stream)
-        hepf.reconstruct_tth(dev, out_idx, n_sel, V, seed, params, out_best=out_best, ws=reco_ws, stream=stream)
-        if ev_mid is not None:
-            ev_mid[1].record(stream)
-        return n_sel
-
-    for _ in range(W):
-        n_sel = step()
-    torch.cuda.synchronize()
-    idx_host = out_idx[:n_sel].cpu().numpy().view(np.uint32)
-    n_solves = solves_of(store, idx_host, V)
+    # weak scaling: rank r owns global events [r n, (r+1) n); the Philox keys use the global index
+    run = TthRun(hepf, binding, cfg, n_ev, rank * n_ev, V, params)
+    store, n, seed = run.store, run.n, cfg.reco_seed
 
     sampler = ClockSampler(local)
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
     sampler.start()
-    hepf.launch_count(reset=True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    mids = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    binding.timing_enable(True)
-    k_search, k_search6, k_final, k_sel, k_sel_eval = [], [], [], [], []
-    e0.record(stream)
-    for s in range(args.steps):
-        step(mids[s])
-        # device time of each kernel of this step, from events the library records on the stream around its launches
-        k_search.append(binding.timing_ms(3, 4)); k_search6.append(binding.timing_ms(4, 5)); k_final.append(binding.timing_ms(5, 6)); k_sel.append(binding.timing_ms(0, 2)); k_sel_eval.append(binding.timing_ms(0, 1))
-    e1.record(stream)
-    torch.cuda.synchronize()
-    binding.timing_enable(False)
-    launches = hepf.launch_count()
+    ms_local = run.measure(args.steps, W, barrier=(dist.barrier if world > 1 else None))
     clocks = sampler.stop()
-    ms_total = e0.elapsed_time(e1)
-    ms_reco = float(np.mean([a.elapsed_time(b) for a, b in mids]))
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    n_sel, n_solves = run.n_sel, run.n_solves
+    t = torch.tensor([run.ms_total], dtype=torch.float64, device="cuda")
     tot = torch.tensor([float(n_solves)], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.barrier()
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    ms_total, all_solves = float(t.item()), float(tot.item())
-    ms_per_step = ms_total / args.steps
+    ms_per_step, all_solves = float(t.item()) / args.steps, float(tot.item())
     value = all_solves / (ms_per_step * 1e-3)
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region --------------
@@ -330,7 +422,9 @@ def main():
     arena = torch.empty(binding.tth_host_arena_bytes(n, V) + 512, dtype=torch.uint8, device="cuda")
     hb = torch.empty((max(n, 1), 128), dtype=torch.uint8).pin_memory()
     hi = torch.empty(max(n, 1), dtype=torch.int32).pin_memory()
-    hepf.tth_host(hstore, cfg.cuts, V, seed, params, arena=arena, out_best=hb, out_idx=hi, stream=stream)
+    stream = run.stream
+    for _ in range(2):
+        hepf.tth_host(hstore, cfg.cuts, V, seed, params, arena=arena, out_best=hb, out_idx=hi, stream=stream)
     e2e_steps = max(1, min(args.steps, 10))
     if world > 1:
         dist.barrier()
@@ -344,16 +438,20 @@ def main():
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
     e2e = {"value": all_solves / float(te.item()), "unit": UNIT,
            "h2d_bytes_per_step": int(64 * store.stride * 8 + n * 4),
-           "d2h_bytes_per_step": int(8 + n_sel * (128 + 4) + 8 * len(cfg.cuts)), "ms_per_step": 1e3 * float(te.item())}
+           "d2h_bytes_per_step": int(8 + n_sel * (128 + 4) + 8 * len(cfg.cuts)), "ms_per_step": 1e3 * float(te.item()),
+           "steps": e2e_steps}
+    del arena, hb, hi, pin_cols, pin_flags, hstore
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    # ---- roofline of the dominant kernel (reco_kernel: FP64-ALU bound) -----------------------------------------------
+    # ---- roofline of the dominant kernel (FP64-ALU bound) and of select (HBM bound) ------------------------------------
+    prof = load_profiled_ops()
     sm_max = clocks.get("sm_max_mhz") or 1965.0
     sms = torch.cuda.get_device_properties(local).multi_processor_count
-    peak_tflops = sms * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    roofline, select_line = run.rooflines(ms_per_step, sm_max, sms, prof)
+    # measured FP64 roof of this box: a register-resident DFMA chain (FMA = 2 flop)
     sink = torch.zeros(1, dtype=torch.float64, device="cuda")
     per_thread = 1 << 20
     binding.fp64_peak_probe(sms * 8, 256, per_thread, sink, stream)
@@ -361,45 +459,43 @@ def main():
     p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     p0.record(stream); binding.fp64_peak_probe(sms * 8, 256, per_thread, sink, stream); p1.record(stream)
     torch.cuda.synchronize()
-    fma_peak = 2.0 * sms * 8 * 256 * per_thread / (p0.elapsed_time(p1) * 1e-3) / 1e12
-    nb6 = float(np.mean(k_search6)) > float(np.mean(k_search))     # which candidate-count class dominates this workload
-    ms_search = float(np.mean(k_search6 if nb6 else k_search))
-    ops = FP64_OPS_PER_SOLVE_NB6 if nb6 else FP64_OPS_PER_SOLVE
-    LANE_OPS_PER_SOLVE = sum(ops.values()); FLOP_PER_SOLVE = ops["dadd"] + ops["dmul"] + 2.0 * ops["dfma"]
-    achieved = FLOP_PER_SOLVE * n_solves / (ms_search * 1e-3) / 1e12
-    lane_rate = LANE_OPS_PER_SOLVE * n_solves / (ms_search * 1e-3)
-    lane_peak = sms * FP64_LANES_PER_SM * sm_max * 1e6
-    # ALU-bound: the unit of work is one FP64 pipe instruction per lane (DADD, DMUL or DFMA), the peak is the pipe's issue
-    # rate 148 SMs x 64 lanes x clock (DESIGN.md 6.2 / 7); the FMA = 2 flop figures are given beside it
-    roofline = {"bound": "alu", "kernel": "reco_search_kernel<16,6>" if nb6 else "reco_search_kernel<16,4>",
-                "achieved": lane_rate / 1e12, "peak": lane_peak / 1e12, "unit": "T FP64 lane-op/s",
-                "frac": lane_rate / lane_peak, "traffic": DRAM_BYTES_PER_LAUNCH if args.workload == "cfg2" else None,
-                "peak_source": f"{sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max:.0f} MHz (DESIGN.md section 6.2)",
-                "fp64_lane_ops_per_solve": LANE_OPS_PER_SOLVE, "flop_per_solve": FLOP_PER_SOLVE,
-                "tflops_fma2": achieved, "tflops_fma2_peak": peak_tflops, "dfma_chain_measured_tflops": fma_peak,
-                "ncu_sm__pipe_fp64_cycles_active_pct": None if nb6 or args.workload != "cfg2" else 50.0,
-                "kernel_ms": ms_search, "kernel_share_of_step": ms_search / ms_per_step,
-                "other_kernels_ms": {"reco_search_other_class": float(np.mean(k_search if nb6 else k_search6)),
-                                     "select_eval+scatter": float(np.mean(k_sel)), "reco_finalize": float(np.mean(k_final)),
-                                     "hepf_reconstruct_tth_call": ms_reco}}
-    sel_bytes = chain_bytes_per_event(cfg.cuts) * n + 4 * n_sel
-    sel_ms = float(np.mean(k_sel_eval))
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    hbm_peak = float(json.load(open(peaks_path)).get("hbm_gbs", 6650.0)) if os.path.exists(peaks_path) else 6650.0
-    select_line = {"kernel": "select_eval_kernel", "events_per_s": n / (sel_ms * 1e-3), "bound": "hbm",
-                   "achieved": sel_bytes / (sel_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                   "frac": sel_bytes / (sel_ms * 1e-3) / 1e9 / hbm_peak, "algorithmic_bytes": sel_bytes, "kernel_ms": sel_ms,
-                   "eval+scatter_ms": float(np.mean(k_sel))}
+    roofline["dfma_chain_measured_tflops"] = 2.0 * sms * 8 * 256 * per_thread / (p0.elapsed_time(p1) * 1e-3) / 1e12
+    roofline["tflops_fma2_peak"] = sms * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",
            "config": {"workload": cfg.name, "events_per_gpu": n, "selected_per_gpu": n_sel,
-                      "n_variations": V, "pairings": 12 if cfg.n_fake_b == 0 else 30, "variations": V, "solves_per_step": all_solves,
-                      "l2": (f"inputs ({516 * n / 1e6:.0f} MB of columns) larger than the 126 MB L2; no flush needed" if 516 * n > 126e6 else f"inputs ({516 * n / 1e6:.1f} MB) fit in L2: parity-test configuration, not a bench line"),
+                      "n_variations": V, "pairings": 12 if cfg.n_fake_b == 0 else 30, "solves_per_step": all_solves,
+                      "l2": (f"inputs ({516 * n / 1e6:.0f} MB of columns) larger than the 126 MB L2; no flush needed" if 516 * n > 126e6
+                             else f"inputs ({516 * n / 1e6:.1f} MB) fit in L2: parity-test configuration, not a bench line"),
                       "parallelism": f"dp{world} (events sharded by global index, no collective)"},
-           "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "select": select_line}
+           "clocks": clocks, "e2e": e2e, "gpu_launches": run.launches, "roofline": roofline, "select": select_line}
+    idx_host = run.idx_host
     if not args.no_cpu_baseline and world == 1:      # the oracle is timed beside the GPU number on rank 0 at N = 1 only
-        out["cpu_baseline"] = cpu_oracle_rate(store, idx_host, V, seed, chain=cfg.cuts)
+        cores = os.cpu_count() or 1
+        out["cpu_baseline"] = cpu_oracle_rate(store, idx_host, V, seed, cores, target_s=10.0)
+        one = cpu_oracle_rate(store, idx_host, V, seed, 1, target_s=6.0)
+        out["cpu_baseline"]["single_thread"] = {"value": one["value"], "unit": UNIT, "cores": 1, "sample": one["sample"]}
+    # ---- the other configs of BASELINE.json, device-timed in the same run (default workload, one GPU only) ---------------
+    if args.workload == "cfg2" and world == 1 and not args.no_extra_configs and not args.events and not args.variations:
+        run.free()
+        extra = {}
+        for cid in (3, 4):
+            c = hs.CONFIGS[cid]
+            r = TthRun(hepf, binding, c, c.n_events, 0, c.n_variations, None)
+            k = max(3, min(args.steps, 10 if cid == 3 else 20))
+            ms = r.measure(k, 3)
+            roof, sel = r.rooflines(ms, sm_max, sms, prof)
+            extra[f"cfg{cid}"] = {"workload": c.name, "ms_per_step": ms, "steps": k, "value": r.n_solves / (ms * 1e-3), "unit": UNIT,
+                                  "selected": r.n_sel, "solves_per_step": r.n_solves, "roofline": roof, "select": sel}
+            r.free()
+        free, _ = torch.cuda.mem_get_info()
+        n5 = hs.PHILOX_CFG5["n"]
+        if free > 8 * n5 + (1 << 30):
+            p = time_philox(hepf, n5, max(3, min(args.steps, 10)), 3)
+            extra["cfg5"] = {"workload": p["workload"], "ms_per_step": p["ms_per_step"], "value": p["value"], "unit": p["unit"],
+                             "roofline": p["roofline"]}
+        out["configs"] = extra
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

@@ -80,7 +80,8 @@ typedef struct {
 /* Best solution of one event ("the one with highest probability is considered to be the correct
  * solution"; "only the highest probable solution was considered").  128 bytes.
  * status bits: 1 = has a solution; 2 = not applicable (n_lep != 2, same-sign, < 4 b candidates);
- *              4 = more than 6 b candidates, truncated to the 6 lowest slots.
+ *              4 = more than 6 b candidates, truncated to the 6 lowest slots;
+ *              8 = idx[k] >= n_events (the entry is treated as not applicable: bits 2 and 8, NaN / -1 payload).
  * Without a solution the floating-point payload is NaN and the integer payload is -1 (the paper's "discards the
  * event if no solution was found"). */
 typedef struct {
@@ -111,7 +112,8 @@ size_t hepf_select_workspace_bytes(int64_t n_events);
  * candidates solve the dileptonic ttbar kinematics (two leg conics -> quartic; Ferrari closed form + Newton
  * polish, FP64), score every solution (Higgs pair mass term + neutrino pT term) and keep the best over
  * variations x pairings x Higgs pairs x roots (§4; definition: DESIGN.md "Method").
- *   idx          device uint32[n_idx]: events to reconstruct (normally hepf_select's out_idx); values < n_events.
+ *   idx          device uint32[n_idx]: events to reconstruct (normally hepf_select's out_idx); an entry >= n_events
+ *                gets status 2 | 8 and no event data is read for it.
  *   n_idx        host value.
  *   host_params  host pointer or NULL.
  *   out_best     device hepf_best_t[n_idx], 16-byte aligned; out_best[k] belongs to idx[k].
@@ -123,6 +125,17 @@ int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t* idx, int64
                          uint64_t seed, const hepf_tth_params_t* host_params, hepf_best_t* out_best, void* ws,
                          size_t ws_bytes, void* stream);
 size_t hepf_reconstruct_workspace_bytes(int64_t n_idx, int32_t n_variations);
+/*
+ * hepf_reconstruct_tth_n — the same operation with the LENGTH OF THE LIST IN DEVICE MEMORY, so that select ->
+ * reconstruct needs no host round trip in the middle of the path (the reconstruction is the last cut of one
+ * pipeline): the kernels read *n_idx_device (normally hepf_select's out_count) when they run, clamped to [0, n_idx_cap].
+ *   n_idx_device device int64, 8-byte aligned;  n_idx_cap host value: capacity of idx / out_best (e.g. n_events);
+ *   ws           >= hepf_reconstruct_workspace_bytes(n_idx_cap, n_variations).   Everything else as above; records
+ *   beyond the device-side length are not written.
+ */
+int hepf_reconstruct_tth_n(const hepf_events_t* events, const uint32_t* idx, const int64_t* n_idx_device, int64_t n_idx_cap,
+                           int32_t n_variations, uint64_t seed, const hepf_tth_params_t* host_params, hepf_best_t* out_best,
+                           void* ws, size_t ws_bytes, void* stream);
 void hepf_default_params(hepf_tth_params_t* host_params);
 
 /*
@@ -137,7 +150,7 @@ int hepf_philox_normal(uint64_t seed, uint64_t counter, uint64_t n, double* out,
 /*
  * hepf_tth_host — the whole path from HOST buffers: copies the columns of `host_events` (a view of HOST
  * memory, pinned for full speed) to the device arena, runs hepf_select and hepf_reconstruct_tth and copies the
- * results back.  Large samples are cut into up to 8 chunks of consecutive events whose copies (two internal copy
+ * results back.  Large samples are cut into up to 10 chunks of consecutive events whose copies (two internal copy
  * streams) overlap the kernels of the neighbouring chunks; the results are byte-identical to the device entry points
  * on one view.  Synchronous: returns when host_out_* are filled.
  *   host_out_idx   host uint32[n_events] or NULL;  host_out_best  host hepf_best_t[n_events] (first n_sel used);

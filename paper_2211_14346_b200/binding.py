@@ -72,6 +72,8 @@ def load():
                                   C.c_void_p, C.c_size_t, C.c_void_p]
         L.hepf_reconstruct_tth.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_int32, C.c_uint64,
                                            C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hepf_reconstruct_tth_n.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_uint64,
+                                             C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.hepf_philox_normal.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p]
         L.hepf_tth_host.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_int32, C.c_uint64,
                                     C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
@@ -148,6 +150,19 @@ class DeviceEvents:
     def view(self) -> _Events:
         return _view(self.cols.data_ptr(), self.flags.data_ptr(), self.n_events, self.stride, self.event_base)
 
+    def subview(self, lo: int, hi: int) -> "DeviceEvents":
+        """Events [lo, hi) of this store as a pointer-offset view (no copy): same columns, event_base + lo, so the records
+        are those of the whole store (the smearing is keyed by the global index).  lo must be a multiple of 4 (16-byte
+        alignment of every column, flags included); use sharding.shard_range for rank boundaries."""
+        if lo % 4 or not 0 <= lo <= hi <= self.n_events:
+            raise HepfError(f"subview [{lo}, {hi}): lo must be a multiple of 4 inside [0, {self.n_events}]")
+        sub = object.__new__(DeviceEvents)
+        sub.cols, sub.flags = self.cols, self.flags
+        sub.n_events, sub.stride, sub.event_base, sub._off = hi - lo, self.stride, self.event_base + lo, getattr(self, "_off", 0) + lo
+        sub.view = lambda: _view(self.cols.data_ptr() + 8 * sub._off, self.flags.data_ptr() + 4 * sub._off, sub.n_events,
+                                 sub.stride, sub.event_base)
+        return sub
+
 
 def select(events: DeviceEvents, chain, *, with_cutflow: bool = True, out_idx=None, out_count=None, out_cutflow=None,
            ws=None, stream=None):
@@ -189,6 +204,25 @@ def reconstruct_tth(events: DeviceEvents, idx, n_idx: int, n_variations: int, se
                                 ws.numel(), _stream_ptr(stream))
     _check(rc, "hepf_reconstruct_tth")
     return out_best[:n_idx]
+
+
+def reconstruct_tth_n(events: DeviceEvents, idx, n_idx_device, n_idx_cap: int, n_variations: int, seed: int,
+                      params: Params | None = None, *, out_best=None, ws=None, stream=None):
+    """hepf_reconstruct_tth_n: the list length is the int64 device tensor `n_idx_device` (hepf_select's out_count); returns
+    the uint8 tensor [n_idx_cap, 128] of which the first n_idx_device records are written.  No host synchronisation."""
+    import torch
+    L = load()
+    if out_best is None:
+        out_best = torch.empty((max(n_idx_cap, 1), 128), dtype=torch.uint8, device=events.cols.device)
+    need = L.hepf_reconstruct_workspace_bytes(max(n_idx_cap, 0), n_variations)
+    if ws is None or ws.numel() < need:
+        ws = torch.empty(max(need, 16), dtype=torch.uint8, device=events.cols.device)
+    ev = events.view()
+    rc = L.hepf_reconstruct_tth_n(C.byref(ev), idx.data_ptr(), n_idx_device.data_ptr(), n_idx_cap, n_variations, seed,
+                                  C.byref(params) if params is not None else None, out_best.data_ptr(), ws.data_ptr(),
+                                  ws.numel(), _stream_ptr(stream))
+    _check(rc, "hepf_reconstruct_tth_n")
+    return out_best
 
 
 def best_to_numpy(out_best) -> np.ndarray:

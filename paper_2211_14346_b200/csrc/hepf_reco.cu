@@ -786,6 +786,13 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   return best_key;
 }
 
+// length of the list: a host value (n_dev == NULL), or read from device memory and clamped to the capacity
+__device__ __forceinline__ int64_t list_length(const int64_t* n_dev, int64_t n_cap) {
+  if (!n_dev) return n_cap;
+  const int64_t n = __ldg(n_dev);
+  return n < 0 ? 0 : (n < n_cap ? n : n_cap);
+}
+
 // Persistent warps: each warp draws the next group of `epc` consecutive list entries from a global counter; its
 // lanes look at one entry each (index, flags), the entries this instantiation owns are then reconstructed one after the
 // other by the whole warp.  NBT = 4 owns the events with exactly four b candidates (and writes the "nothing to do" key
@@ -793,11 +800,13 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
 // for its class.
 template <int VC, int NBT, int RW, int MINB>
 __global__ void __launch_bounds__(32 * RW, MINB)
-reco_search_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, int epc, int V, uint32_t k0, uint32_t k1,
-                   hepf_tth_params_t P, uint2* __restrict__ winners, unsigned long long* __restrict__ next_group) {
+reco_search_kernel(RecoCols ev, const uint32_t* __restrict__ idx, const int64_t* __restrict__ n_dev, int64_t n_cap, int epc, int V,
+                   uint32_t k0, uint32_t k1, hepf_tth_params_t P, uint2* __restrict__ winners,
+                   unsigned long long* __restrict__ next_group) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   WarpMem<VC, NBT>& W = reinterpret_cast<WarpMem<VC, NBT>*>(smem_raw)[threadIdx.x >> 5];
   const int lane = threadIdx.x & 31;
+  const int64_t n_idx = list_length(n_dev, n_cap);
   const int64_t n_groups = (n_idx + epc - 1) / epc;
   for (;;) {
     unsigned long long gq = 0;
@@ -823,12 +832,9 @@ reco_search_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_idx,
   }
 }
 
-// One thread per selected event: re-derive the winner in full and write the record.
-__global__ void __launch_bounds__(128)
-reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, uint32_t k0, uint32_t k1,
-                     hepf_tth_params_t P, const uint2* __restrict__ winners, hepf_best_t* __restrict__ out) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= n_idx) return;
+// One selected event: re-derive the winner in full, polish it and write the record.
+__device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_t* __restrict__ idx, int64_t k, uint32_t k0, uint32_t k1,
+                                               const hepf_tth_params_t& P, const uint2* __restrict__ winners, hepf_best_t* __restrict__ out) {
   const EventHead h = load_head(ev, (int64_t)__ldg(idx + k));
   const uint2 w = winners[k];
   hepf_best_t* o = out + k;
@@ -917,8 +923,17 @@ reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, int64_t n_id
   o->status = h.status | 1u; o->event = (uint32_t)(h.e + ev.out_off);
 }
 
+// One thread per listed event (grid-stride: the grid is sized from the capacity, the length may live on the device).
+__global__ void __launch_bounds__(128)
+reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, const int64_t* __restrict__ n_dev, int64_t n_cap, uint32_t k0,
+                     uint32_t k1, hepf_tth_params_t P, const uint2* __restrict__ winners, hepf_best_t* __restrict__ out) {
+  const int64_t n_idx = list_length(n_dev, n_cap);
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_idx; k += (int64_t)gridDim.x * blockDim.x)
+    finalize_event(ev, idx, k, k0, k1, P, winners, out);
+}
+
 template <int VC, int NBT, int RW, int MINB>
-static int launch_search(const RecoCols& cols, const uint32_t* idx, int64_t n_idx, int V, uint64_t seed,
+static int launch_search(const RecoCols& cols, const uint32_t* idx, const int64_t* n_dev, int64_t n_idx, int V, uint64_t seed,
                          const hepf_tth_params_t& P, uint2* winners, unsigned long long* counter, cudaStream_t stream) {
   const size_t smem = sizeof(WarpMem<VC, NBT>) * RW;
   auto kern = reco_search_kernel<VC, NBT, RW, MINB>;
@@ -941,7 +956,7 @@ static int launch_search(const RecoCols& cols, const uint32_t* idx, int64_t n_id
   const int64_t n_groups = (n_idx + epc - 1) / epc;
   const int64_t want = (n_groups + RW - 1) / RW, cap = (int64_t)sms * blocks_per_sm;
   const unsigned grid = (unsigned)(want < cap ? want : cap);
-  kern<<<grid, 32 * RW, smem, stream>>>(cols, idx, n_idx, epc, V, (uint32_t)seed, (uint32_t)(seed >> 32), P, winners, counter);
+  kern<<<grid, 32 * RW, smem, stream>>>(cols, idx, n_dev, n_idx, epc, V, (uint32_t)seed, (uint32_t)(seed >> 32), P, winners, counter);
   count_launch();
   HEPF_CUDA_TRY(cudaGetLastError());
   return HEPF_OK;
@@ -949,15 +964,15 @@ static int launch_search(const RecoCols& cols, const uint32_t* idx, int64_t n_id
 
 // both candidate-count classes: n_b = 4 (tables for 4 candidates, more warps per SM) and n_b = 5, 6
 template <int VC4, int VC6, int RW, int MINB4, int MINB6>
-static int launch_search_both(const RecoCols& cols, const uint32_t* idx, int64_t n_idx, int V, uint64_t seed,
+static int launch_search_both(const RecoCols& cols, const uint32_t* idx, const int64_t* n_dev, int64_t n_idx, int V, uint64_t seed,
                               const hepf_tth_params_t& P, uint2* winners, cudaStream_t stream) {
   unsigned long long* counters = reinterpret_cast<unsigned long long*>(winners + n_idx);   // two group counters
   HEPF_CUDA_TRY(cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), stream));
   timing_mark(T_RECO0, stream);
-  int rc = launch_search<VC4, 4, RW, MINB4>(cols, idx, n_idx, V, seed, P, winners, counters, stream);
+  int rc = launch_search<VC4, 4, RW, MINB4>(cols, idx, n_dev, n_idx, V, seed, P, winners, counters, stream);
   timing_mark(T_RECO1, stream);
   if (rc != HEPF_OK) return rc;
-  rc = launch_search<VC6, 6, RW, MINB6>(cols, idx, n_idx, V, seed, P, winners, counters + 1, stream);
+  rc = launch_search<VC6, 6, RW, MINB6>(cols, idx, n_dev, n_idx, V, seed, P, winners, counters + 1, stream);
   timing_mark(T_RECO2, stream);
   return rc;
 }
@@ -975,11 +990,19 @@ extern "C" size_t hepf_reconstruct_workspace_bytes(int64_t n_idx, int32_t n_vari
 extern "C" int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
                                     uint64_t seed, const hepf_tth_params_t* host_params, hepf_best_t* out_best, void* ws,
                                     size_t ws_bytes, void* stream_) {
-  return hepf::reconstruct_impl(events, idx, n_idx, n_variations, seed, host_params, out_best, ws, ws_bytes,
+  return hepf::reconstruct_impl(events, idx, nullptr, n_idx, n_variations, seed, host_params, out_best, ws, ws_bytes,
                                 (cudaStream_t)stream_, 0);
 }
 
-int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int32_t n_variations, uint64_t seed,
+extern "C" int hepf_reconstruct_tth_n(const hepf_events_t* events, const uint32_t* idx, const int64_t* n_idx_device, int64_t n_idx_cap,
+                                      int32_t n_variations, uint64_t seed, const hepf_tth_params_t* host_params,
+                                      hepf_best_t* out_best, void* ws, size_t ws_bytes, void* stream_) {
+  if (!n_idx_device || !aligned(n_idx_device, 8)) { set_error("hepf_reconstruct_tth_n: n_idx_device NULL or misaligned"); return HEPF_ERR_ARG; }
+  return hepf::reconstruct_impl(events, idx, n_idx_device, n_idx_cap, n_variations, seed, host_params, out_best, ws, ws_bytes,
+                                (cudaStream_t)stream_, 0);
+}
+
+int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, const int64_t* n_dev, int64_t n_idx, int32_t n_variations, uint64_t seed,
                            const hepf_tth_params_t* host_params, hepf_best_t* out_best, void* ws, size_t ws_bytes,
                            cudaStream_t stream, int64_t event_out_offset) {
   int rc = check_events(events);
@@ -1002,12 +1025,15 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, int
                       events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags,
                       events->n_events, events->stride, events->event_base, event_out_offset};
   uint2* winners = reinterpret_cast<uint2*>(ws);
-  if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 12, 10>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
-  else rc = launch_search_both<16, 16, 2, 10, 7>(cols, idx, n_idx, n_variations, seed, P, winners, stream);
+  if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 12, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
+  else rc = launch_search_both<16, 8, 2, 10, 9>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
   if (rc != HEPF_OK) return rc;
-  const int64_t fblocks = (n_idx + 127) / 128;
-  reco_finalize_kernel<<<(unsigned)fblocks, 128, 0, stream>>>(cols, idx, n_idx, (uint32_t)seed, (uint32_t)(seed >> 32), P,
-                                                             winners, out_best);
+  int dev = 0, sms = 148;
+  HEPF_CUDA_TRY(cudaGetDevice(&dev));
+  HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int64_t want = (n_idx + 127) / 128, cap = (int64_t)sms * 32;
+  reco_finalize_kernel<<<(unsigned)(want < cap ? want : cap), 128, 0, stream>>>(cols, idx, n_dev, n_idx, (uint32_t)seed,
+                                                                             (uint32_t)(seed >> 32), P, winners, out_best);
   count_launch();
   timing_mark(T_RECO3, stream);
   HEPF_CUDA_TRY(cudaGetLastError());

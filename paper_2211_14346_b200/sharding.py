@@ -10,13 +10,14 @@ from __future__ import annotations
 
 
 def shard_range(n_events: int, rank: int, world: int) -> tuple[int, int]:
-    """Contiguous range [lo, hi) of rank `rank`.  The unit is a PAIR of events, so every boundary is even and a slice
-    of an even-stride SoA store keeps its 16-byte row alignment; sizes differ by at most three events."""
-    pairs = (n_events + 1) // 2
-    base, rem = divmod(pairs, world)
+    """Contiguous range [lo, hi) of rank `rank`.  The unit is FOUR events, so every boundary is a multiple of 4: a
+    pointer-offset view of a resident store (DeviceEvents.subview) then keeps the 16-byte alignment hepf_events_t asks
+    of every column, the 4-byte flags column included; sizes differ by at most seven events."""
+    quads = (n_events + 3) // 4
+    base, rem = divmod(quads, world)
     lo = rank * base + min(rank, rem)
     hi = lo + base + (1 if rank < rem else 0)
-    return min(2 * lo, n_events), min(2 * hi, n_events)
+    return min(4 * lo, n_events), min(4 * hi, n_events)
 
 
 def global_survivor_offset(local_count: int, group=None, device="cpu") -> tuple[int, int]:

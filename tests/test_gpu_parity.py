@@ -57,6 +57,18 @@ def test_philox_normal_ragged_ranges_and_alignment(hepf, counter, n, offset):
     assert (got[:offset] == -7.0).all() and (got[offset + n:] == -7.0).all()     # nothing written outside
 
 
+def test_philox_normal_many_normals_far_into_the_stream(hepf):
+    """2^26 normals starting at 3 * 2^40 + 1 (odd start, unaligned path for the first element): bit for bit against the
+    oracle.  The kernel's division and square root are hand-written correctly rounded cores (hepf_common.cuh), the oracle's
+    are the host's IEEE operations: 3.3e7 divisions and square roots of exactly the operand domains in question."""
+    import torch
+    n, start = 1 << 26, 3 * (1 << 40) + 1
+    got = hepf.philox_normal(12345678901234567, start, n)
+    torch.cuda.synchronize()
+    want = oracle.philox_normal(12345678901234567, start, n)
+    assert got.cpu().numpy().tobytes() == want.tobytes()
+
+
 def test_philox_normal_split_invariance(hepf):
     import torch
     a = hepf.philox_normal(7, 10, 100_003).cpu().numpy()
@@ -220,6 +232,65 @@ def test_tth_host_equals_device_path(hepf):
     hidx, hbest, hcf = hepf.tth_host(st, cfg.cuts, 8, 42)
     assert np.array_equal(hidx, idx) and np.array_equal(hcf, cf)
     assert hbest.tobytes() == want.tobytes()
+
+
+def test_device_side_list_length_equals_host_side(hepf):
+    """hepf_reconstruct_tth_n reads the list length from device memory (hepf_select's out_count): same bytes as the host-n
+    call, nothing written beyond the length, no host synchronisation between select and reconstruct; a count larger than
+    the capacity is clamped, zero writes nothing."""
+    import torch
+    st = hs.generate(5003, 17, with_truth=False)
+    dev = hepf.DeviceEvents.from_host(st)
+    idx_t, count, _ = hepf.select(dev, hs.CHAIN_BASE)
+    out = torch.full((st.n_events, 128), 0x5A, dtype=torch.uint8, device="cuda")
+    hepf.reconstruct_tth_n(dev, idx_t, count, st.n_events, 24, 7, out_best=out)
+    torch.cuda.synchronize()
+    n = int(count.item())
+    want = hepf.reconstruct_tth(dev, idx_t, n, 24, 7)
+    torch.cuda.synchronize()
+    assert 1000 < n < st.n_events and torch.equal(out[:n], want)
+    assert bool((out[n:] == 0x5A).all())
+    big = torch.tensor([10 ** 9], dtype=torch.int64, device="cuda")
+    out2 = torch.full((n + 5, 128), 0x5A, dtype=torch.uint8, device="cuda")
+    hepf.reconstruct_tth_n(dev, idx_t, big, n, 24, 7, out_best=out2)         # clamped to the capacity n
+    zero = torch.zeros(1, dtype=torch.int64, device="cuda")
+    out3 = torch.full((n, 128), 0x5A, dtype=torch.uint8, device="cuda")
+    hepf.reconstruct_tth_n(dev, idx_t, zero, n, 24, 7, out_best=out3)
+    torch.cuda.synchronize()
+    assert torch.equal(out2[:n], want) and bool((out2[n:] == 0x5A).all()) and bool((out3 == 0x5A).all())
+
+
+def test_subview_at_a_shard_boundary_and_out_of_range_indices(hepf):
+    """(a) A pointer-offset view of a resident store at sharding.shard_range's boundaries (multiples of 4 events: 16-byte
+    alignment of every column, flags included) gives the records of the whole store.  (b) idx[k] >= n_events is answered
+    with status 2 | 8 and the NaN / -1 payload, and does not disturb its neighbours."""
+    import torch
+    from paper_2211_14346_b200 import sharding
+    from paper_2211_14346_b200.binding import best_to_numpy
+    st = hs.generate(3001, 23, with_truth=False)
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, hs.CHAIN_BASE)
+    whole = _gpu_reco(hepf, dev, idx_t, n, 12, 5)
+    parts = []
+    for r in range(3):
+        lo, hi = sharding.shard_range(st.n_events, r, 3)
+        assert lo % 4 == 0
+        sub = dev.subview(lo, hi)
+        i2, c2, _ = hepf.select(sub, hs.CHAIN_BASE)
+        torch.cuda.synchronize()
+        rec = best_to_numpy(hepf.reconstruct_tth(sub, i2, int(c2.item()), 12, 5)).copy()
+        rec["event"] += lo
+        parts.append(rec)
+    assert np.concatenate(parts).tobytes() == whole.tobytes()
+    with pytest.raises(hepf.HepfError):
+        dev.subview(2, 100)
+    bad = idx.copy().astype(np.uint32)
+    bad[5] = st.n_events; bad[77] = 0xFFFFFFFF
+    bad_t = torch.from_numpy(bad.view(np.int32)).cuda()
+    got = _gpu_reco(hepf, dev, bad_t, n, 12, 5)
+    for k in (5, 77):
+        assert got["status"][k] == 10 and np.isnan(got["loglik"][k]) and got["variation"][k] == -1 and got["event"][k] == bad[k]
+    keep = np.ones(n, bool); keep[[5, 77]] = False
+    assert got[keep].tobytes() == whole[keep].tobytes()
 
 
 def test_reconstruct_rejects_bad_arguments(hepf):

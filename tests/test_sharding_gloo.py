@@ -38,15 +38,15 @@ def _worker(rank, world, port, n_events, tmp):
     dist.destroy_process_group()
 
 
-def test_shard_range_covers_everything_with_even_boundaries():
+def test_shard_range_covers_everything_with_16_byte_aligned_boundaries():
     from paper_2211_14346_b200.sharding import shard_range
     for n in (0, 1, 2, 7, 10, 1001, 20_000_000):
         for w in (1, 2, 3, 4, 8):
             r = [shard_range(n, k, w) for k in range(w)]
             assert r[0][0] == 0 and r[-1][1] == n
             for a, b in zip(r, r[1:]):
-                assert a[1] == b[0] and (b[0] % 2 == 0 or b[0] == n)
-            assert max(h - l for l, h in r) - min(h - l for l, h in r) <= 3
+                assert a[1] == b[0] and (b[0] % 4 == 0 or b[0] == n)     # flags column: 4 events = 16 bytes
+            assert max(h - l for l, h in r) - min(h - l for l, h in r) <= 7
 
 
 @pytest.mark.timeout(300)
