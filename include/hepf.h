@@ -65,7 +65,8 @@ typedef enum {
   HEPF_CUT_NBJET_GE = 6,      /* same, b-tagged jets only                              */
   HEPF_CUT_MET_GT = 7,        /* met > lo                                              */
   HEPF_CUT_MLL_GT = 8,        /* mll > lo                                              */
-  HEPF_CUT_MLL_OUTSIDE = 9    /* mll < lo or mll > hi                                  */
+  HEPF_CUT_MLL_OUTSIDE = 9,   /* mll < lo or mll > hi                                  */
+  HEPF_CUT_MET_GT_RECORD = 10 /* met > lo; on passing writes the derived variable met * hi (hepf_select_record) */
 } hepf_cut_kind_t;
 typedef struct { uint32_t kind; uint32_t n; double lo, hi; } hepf_cut_t;
 
@@ -104,6 +105,18 @@ typedef struct {
 int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
                 int64_t* out_count, int64_t* out_cutflow, void* ws, size_t ws_bytes, void* stream);
 size_t hepf_select_workspace_bytes(int64_t n_events);
+/*
+ * hepf_select_record — hepf_select for a chain that holds one RECORDING cut (section 6.1: a cut may
+ * write a new per-event variable when it passes; the paper's example is "if (met_met <= 30000.) return false; else
+ * { ETmis = met_met; ETmis *= 1.05; return true; }").  HEPF_CUT_MET_GT_RECORD is that cut: it passes if met > lo and then
+ * sets the derived variable of the event to met * hi (one IEEE multiplication).  Events that fail it, or an earlier cut, keep
+ * `derived_default` ("for levels where the information was not yet updated, their default value is used").
+ *   out_derived  device double[n_events], 16-byte aligned: the derived column (the paper's ETmis), one value per event.
+ * In hepf_select the same cut kind only filters.  At most one recording cut per chain.
+ */
+int hepf_select_record(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
+                       int64_t* out_count, int64_t* out_cutflow, double* out_derived, double derived_default, void* ws,
+                       size_t ws_bytes, void* stream);
 
 /*
  * hepf_reconstruct_tth — for each listed event: for every smearing variation v < n_variations draw ten
@@ -199,6 +212,25 @@ typedef enum {
 } hepf_hist_field_t;
 int hepf_histogram(const hepf_best_t* best, int64_t n, int field, double lo, double hi, int32_t nbins, uint64_t* out,
                    void* stream);
+
+/*
+ * hepf_tth_system — the two quantities the paper's example analysis histograms (App. 8.2 listing:
+ * "TLorentzVector ttH = Top + Tbar + Higgs; mTTH = ttH.M(); ptTTH = ttH.Pt();"): invariant mass and transverse momentum of
+ * the reconstructed ttH system of each record, i.e. of l+ + l- + nu + nubar + b + bbar + h1 + h2 with the smeared objects
+ * of the record's variation and E_nu = |p_nu|; m = sqrt(max(E^2 - |p|^2, 0)), pT = sqrt(px^2 + py^2), every operation one
+ * IEEE operation in that order.  The reconstruction being the last cut, these are per-event variables written by a cut
+ * (PAPER.md:278).   best: device hepf_best_t[n] (hepf_reconstruct_tth's output on the same view, seed and parameters);
+ * out: device double[2 n], 16-byte aligned: out[2k] = m_ttH, out[2k+1] = pT_ttH of record k; NaN for a record without solution.
+ */
+int hepf_tth_system(const hepf_events_t* events, const hepf_best_t* best, int64_t n, uint64_t seed,
+                    const hepf_tth_params_t* host_params, double* out, void* stream);
+/*
+ * hepf_histogram_values — hepf_histogram's binning for a plain device column of doubles (a derived per-event variable:
+ * hepf_select_record's ETmis column, hepf_tth_system's m_ttH or pT_ttH): element k is values[k * stride]; every value is
+ * filled except NaN ("no value").   out: device uint64[nbins + 2], zeroed by the call.
+ */
+int hepf_histogram_values(const double* values, int64_t stride, int64_t n, double lo, double hi, int32_t nbins, uint64_t* out,
+                          void* stream);
 
 /* Kernel launches enqueued by this thread's calls since the last reset (bench.py's `gpu_launches`). */
 int64_t hepf_launch_count(int reset);

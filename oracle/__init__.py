@@ -71,6 +71,9 @@ def lib():
         L.orc_philox_normal.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.c_void_p]
         L.orc_philox_normal.restype = None
         L.orc_select.argtypes = [C.POINTER(Events), C.POINTER(Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_select_record.argtypes = [C.POINTER(Events), C.POINTER(Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]
+        L.orc_tth_system.argtypes = [C.POINTER(Events), C.c_void_p, C.c_int64, C.c_uint64, C.POINTER(Params), C.c_void_p]
+        L.orc_histogram_values.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_int32, C.c_void_p]
         L.orc_reconstruct_tth.argtypes = [C.POINTER(Events), C.c_void_p, C.c_int64, C.c_int32, C.c_uint64,
                                           C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_int]
         L.orc_solve_pairing.argtypes = [C.c_void_p] * 6 + [C.c_int, C.POINTER(Params), C.POINTER(Pairing)]
@@ -146,6 +149,41 @@ def select(store, chain):
     if rc != 0:
         raise RuntimeError(f"orc_select: {rc}")
     return idx[: int(count[0])].copy(), cutflow[: len(chain)].copy()
+
+
+def select_record(store, chain, derived_default: float = 0.0):
+    """(idx, cutflow, derived column) of a chain that may hold a recording cut (kind 10 = MET_GT_RECORD: met > lo, writes met * hi)."""
+    ev = events_view(store)
+    idx = np.empty(store.n_events, dtype=np.uint32)
+    count = np.zeros(1, dtype=np.int64)
+    cutflow = np.zeros(max(1, len(chain)), dtype=np.int64)
+    derived = np.empty(store.n_events, dtype=np.float64)
+    rc = lib().orc_select_record(C.byref(ev), make_cuts(chain), len(chain), idx.ctypes.data, count.ctypes.data,
+                                 cutflow.ctypes.data, derived.ctypes.data, derived_default)
+    if rc != 0:
+        raise RuntimeError(f"orc_select_record: {rc}")
+    return idx[: int(count[0])].copy(), cutflow[: len(chain)].copy(), derived
+
+
+def tth_system(store, best, seed: int, params: Params | None = None) -> np.ndarray:
+    """(n, 2) array: invariant mass and transverse momentum of the reconstructed ttH system of each record (NaN if unsolved)."""
+    ev = events_view(store)
+    best = np.ascontiguousarray(best)
+    out = np.empty((len(best), 2), dtype=np.float64)
+    rc = lib().orc_tth_system(C.byref(ev), best.ctypes.data, len(best), seed, C.byref(params) if params is not None else None,
+                              out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_tth_system: {rc}")
+    return out
+
+
+def histogram_values(values: np.ndarray, lo: float, hi: float, nbins: int) -> np.ndarray:
+    v = np.ascontiguousarray(values, dtype=np.float64)
+    out = np.zeros(nbins + 2, dtype=np.uint64)
+    rc = lib().orc_histogram_values(v.ctypes.data, 1, len(v), lo, hi, nbins, out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_histogram_values: {rc}")
+    return out
 
 
 def reconstruct_tth(store, idx, n_variations: int, seed: int, params: Params | None = None, n_threads: int = 1):

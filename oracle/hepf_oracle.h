@@ -46,7 +46,7 @@ typedef struct {
 
 typedef struct { uint32_t kind, n; double lo, hi; } orc_cut_t;
 enum { ORC_NLEP_EQ = 1, ORC_LEP_OS, ORC_LEP_PT_GT, ORC_LEP_ABSETA_LT, ORC_NJET_GE, ORC_NBJET_GE, ORC_MET_GT,
-       ORC_MLL_GT, ORC_MLL_OUTSIDE };
+       ORC_MLL_GT, ORC_MLL_OUTSIDE, ORC_MET_GT_RECORD };
 
 typedef struct {
   double m_top, m_w, m_higgs, sigma_higgs, lambda_nu, lep_sigma, jet_stoch, jet_const, sigma_scale, s_min;
@@ -90,6 +90,9 @@ void orc_philox_normal(uint64_t seed, uint64_t counter, uint64_t n, double* out)
 /* O3 */
 int orc_select(const orc_events_t* ev, const orc_cut_t* cuts, int n_cuts, uint32_t* out_idx, int64_t* out_count,
                int64_t* out_cutflow);
+/* a chain with a recording cut (ORC_MET_GT_RECORD): see oracle_select.cpp */
+int orc_select_record(const orc_events_t* ev, const orc_cut_t* cuts, int n_cuts, uint32_t* out_idx, int64_t* out_count,
+                      int64_t* out_cutflow, double* out_derived, double derived_default);
 /* O4: n_threads > 1 only distributes whole events over OpenMP threads; per-event arithmetic is unchanged */
 int orc_reconstruct_tth(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
                         uint64_t seed, const orc_params_t* params, orc_best_t* out_best, orc_aux_t* out_aux,
@@ -121,6 +124,12 @@ int orc_chi2_semilep(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx,
 
 /* histogram of a field of the records (oracle_hist.cpp; pin: numpy restatement + hand-built edge cases) */
 int orc_histogram(const orc_best_t* best, int64_t n, int field, double lo, double hi, int32_t nbins, uint64_t* out);
+
+/* invariant mass and transverse momentum of the reconstructed ttH system of each record (oracle_reco.cpp), out[2k], out[2k+1] */
+int orc_tth_system(const orc_events_t* ev, const orc_best_t* best, int64_t n, uint64_t seed, const orc_params_t* params,
+                   double* out);
+/* histogram of a plain column of doubles with the rules of orc_histogram (NaN not counted, every value filled) */
+int orc_histogram_values(const double* values, int64_t stride, int64_t n, double lo, double hi, int32_t nbins, uint64_t* out);
 
 #ifdef __cplusplus
 }

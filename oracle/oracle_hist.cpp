@@ -41,3 +41,20 @@ extern "C" int orc_histogram(const orc_best_t* best, int64_t n, int field, doubl
   }
   return 0;
 }
+
+// The same binning for a plain column of doubles, element k at values[k * stride]: the per-event variables a cut or the
+// reconstruction wrote (ETmis, m_ttH, pT_ttH: PAPER.md:278-295, :410-442).  Every finite value is filled; NaN marks "no value".
+extern "C" int orc_histogram_values(const double* values, int64_t stride, int64_t n, double lo, double hi, int32_t nbins,
+                                    uint64_t* out) {
+  if (n < 0 || nbins < 1 || !(hi > lo) || stride < 1 || !out || (n > 0 && !values)) return -1;
+  for (int i = 0; i < nbins + 2; i++) out[i] = 0;
+  const double inv_w = (double)nbins / (hi - lo);
+  for (int64_t k = 0; k < n; k++) {
+    const double t = (values[k * stride] - lo) * inv_w;
+    if (t != t) continue;
+    if (t < 0.0) out[0]++;
+    else if (t >= (double)nbins) out[nbins + 1]++;
+    else out[1 + (int)t]++;
+  }
+  return 0;
+}

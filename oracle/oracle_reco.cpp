@@ -444,3 +444,33 @@ extern "C" int orc_eval_cell(const orc_events_t* ev, uint32_t e, int32_t v, int3
   out->n_higgs = h;
   return 0;
 }
+
+// PAPER.md:410-442 (App. 8.2 listing): "TLorentzVector ttH = Top + Tbar + Higgs; mTTH = ttH.M(); ptTTH = ttH.Pt();" — the
+// invariant mass and the transverse momentum of the reconstructed ttH system, the two quantities the example analysis
+// histograms.  For a record with a solution: the smeared objects of the record's variation (O4 step 2), the neutrinos with
+// E = |p|, and the eight four-vectors added in the order l+, l-, nu, nubar, b, bbar, h1, h2; m = sqrt(max(E^2 - |p|^2, 0)),
+// pT = sqrt(px^2 + py^2).  Without a solution both are NaN.  Every operation is one IEEE operation in the order written.
+extern "C" int orc_tth_system(const orc_events_t* ev, const orc_best_t* best, int64_t n, uint64_t seed,
+                              const orc_params_t* params, double* out) {
+  if (!ev || n < 0 || (n > 0 && (!best || !out))) return -1;
+  orc_params_t P; if (params) P = *params; else orc_default_params(&P);
+  for (int64_t k = 0; k < n; k++) {
+    const orc_best_t& b = best[k];
+    out[2 * k] = out[2 * k + 1] = NaN;
+    if (!(b.status & 1u) || b.event >= (uint64_t)ev->n_events) continue;
+    EventObjects o = load_event(ev, b.event);
+    double s[10], Mx, My; smear(o, b.variation, seed, P, s, &Mx, &My);
+    auto jet = [&](int slot) { return scaled(o.jet[slot], s[2 + slot]); };
+    V4 nu{b.nu[0], b.nu[1], b.nu[2], std::sqrt(b.nu[0] * b.nu[0] + b.nu[1] * b.nu[1] + b.nu[2] * b.nu[2])};
+    V4 nb{b.nubar[0], b.nubar[1], b.nubar[2],
+          std::sqrt(b.nubar[0] * b.nubar[0] + b.nubar[1] * b.nubar[1] + b.nubar[2] * b.nubar[2])};
+    const V4 parts[8] = {scaled(o.lep[o.lp_slot], s[o.lp_slot]), scaled(o.lep[o.lm_slot], s[o.lm_slot]), nu, nb,
+                         jet(b.jet_b), jet(b.jet_bbar), jet(b.jet_h1), jet(b.jet_h2)};
+    V4 sum = parts[0];
+    for (int i = 1; i < 8; i++) { sum.x = sum.x + parts[i].x; sum.y = sum.y + parts[i].y; sum.z = sum.z + parts[i].z; sum.e = sum.e + parts[i].e; }
+    double m2 = sum.e * sum.e - (sum.x * sum.x + sum.y * sum.y + sum.z * sum.z);
+    out[2 * k] = std::sqrt(m2 > 0.0 ? m2 : 0.0);
+    out[2 * k + 1] = std::sqrt(sum.x * sum.x + sum.y * sum.y);
+  }
+  return 0;
+}

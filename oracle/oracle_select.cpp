@@ -32,6 +32,7 @@ static bool pass_cut(const orc_events_t* ev, int64_t i, const orc_cut_t& c) {
       return count >= (int)c.n;
     }
     case ORC_MET_GT: return ev->met[i] > c.lo;
+    case ORC_MET_GT_RECORD: return ev->met[i] > c.lo;   // the side effect is in orc_select_record
     case ORC_MLL_GT: return ev->mll[i] > c.lo;
     case ORC_MLL_OUTSIDE: return ev->mll[i] < c.lo || ev->mll[i] > c.hi;
     default: return false;  // unknown kind: nothing passes
@@ -48,6 +49,30 @@ extern "C" int orc_select(const orc_events_t* ev, const orc_cut_t* cuts, int n_c
     for (int c = 0; c < n_cuts && alive; c++) {
       alive = pass_cut(ev, i, cuts[c]);
       if (alive && out_cutflow) out_cutflow[c]++;  // cutflow[c] = events that passed cuts 0..c
+    }
+    if (alive) { if (out_idx) out_idx[n] = (uint32_t)i; n++; }
+  }
+  if (out_count) *out_count = n;
+  return 0;
+}
+
+// PAPER.md:278-295 (§6.1 listing): a cut may write a new per-event variable when it passes — the paper's example is the
+// missing-E_T cut, "if (met_met <= 30000.) return false; else { ETmis = met_met; ETmis *= 1.05; return true; }" — and
+// such a variable holds a default value "for levels where the information was not yet updated".
+// ORC_MET_GT_RECORD is that cut: met > lo, and on passing derived[i] = met * hi (one rounded multiplication); an event
+// that does not reach the cut, or fails it, keeps derived_default.  Everything else is orc_select.
+extern "C" int orc_select_record(const orc_events_t* ev, const orc_cut_t* cuts, int n_cuts, uint32_t* out_idx,
+                                 int64_t* out_count, int64_t* out_cutflow, double* out_derived, double derived_default) {
+  if (!ev || n_cuts < 0 || n_cuts > 32 || (n_cuts > 0 && !cuts)) return -1;
+  int64_t n = 0;
+  if (out_cutflow) for (int c = 0; c < n_cuts; c++) out_cutflow[c] = 0;
+  for (int64_t i = 0; i < ev->n_events; i++) {
+    if (out_derived) out_derived[i] = derived_default;
+    bool alive = true;
+    for (int c = 0; c < n_cuts && alive; c++) {
+      alive = pass_cut(ev, i, cuts[c]);
+      if (alive && cuts[c].kind == ORC_MET_GT_RECORD && out_derived) out_derived[i] = ev->met[i] * cuts[c].hi;
+      if (alive && out_cutflow) out_cutflow[c]++;
     }
     if (alive) { if (out_idx) out_idx[n] = (uint32_t)i; n++; }
   }

@@ -80,6 +80,10 @@ def load():
                                     C.c_size_t, C.c_void_p]
         L.hepf_chi2_semilep.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.hepf_histogram.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
+        L.hepf_select_record.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                         C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hepf_tth_system.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_uint64, C.POINTER(Params), C.c_void_p, C.c_void_p]
+        L.hepf_histogram_values.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
         L.hepf_timing_enable.argtypes = [C.c_int]
         L.hepf_timing_ms.restype = C.c_double
         L.hepf_timing_ms.argtypes = [C.c_int, C.c_int]
@@ -186,6 +190,51 @@ def select(events: DeviceEvents, chain, *, with_cutflow: bool = True, out_idx=No
                        out_cutflow.data_ptr() if with_cutflow else None, ws.data_ptr(), ws.numel(), _stream_ptr(stream))
     _check(rc, "hepf_select")
     return out_idx, out_count, (out_cutflow[: len(chain)] if with_cutflow else None)
+
+
+def select_record(events: DeviceEvents, chain, derived_default: float = 0.0, *, with_cutflow: bool = True, ws=None, stream=None):
+    """hepf_select_record: (out_idx, out_count, cutflow or None, derived) — derived is the float64 column [n_events] the
+    chain's HEPF_CUT_MET_GT_RECORD cut writes (met * hi for the events that pass it, derived_default for the others)."""
+    import torch
+    L = load()
+    dev = events.cols.device
+    n = events.n_events
+    out_idx = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    out_count = torch.zeros(1, dtype=torch.int64, device=dev)
+    out_cutflow = torch.zeros(max(len(chain), 1), dtype=torch.int64, device=dev) if with_cutflow else None
+    derived = torch.empty(max(n, 2), dtype=torch.float64, device=dev)
+    need = L.hepf_select_workspace_bytes(n)
+    if ws is None or ws.numel() < need:
+        ws = torch.empty(max(need, 16), dtype=torch.uint8, device=dev)
+    ev = events.view()
+    rc = L.hepf_select_record(C.byref(ev), make_cuts(chain), len(chain), out_idx.data_ptr(), out_count.data_ptr(),
+                              out_cutflow.data_ptr() if with_cutflow else None, derived.data_ptr(), derived_default,
+                              ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc, "hepf_select_record")
+    return out_idx, out_count, (out_cutflow[: len(chain)] if with_cutflow else None), derived[:n]
+
+
+def tth_system(events: DeviceEvents, best, n: int, seed: int, params: Params | None = None, *, out=None, stream=None):
+    """hepf_tth_system: float64 tensor [n, 2] = (m_ttH, pT_ttH) of each record of `best` (NaN where there is no solution)."""
+    import torch
+    if out is None:
+        out = torch.empty((max(n, 1), 2), dtype=torch.float64, device=best.device)
+    ev = events.view()
+    rc = load().hepf_tth_system(C.byref(ev), best.data_ptr(), n, seed, C.byref(params) if params is not None else None,
+                                out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "hepf_tth_system")
+    return out[:n]
+
+
+def histogram_values(values, lo: float, hi: float, nbins: int, *, out=None, stream=None):
+    """hepf_histogram_values of a 1-D float64 device tensor (any stride): int64 tensor [nbins + 2]."""
+    import torch
+    if out is None:
+        out = torch.empty(nbins + 2, dtype=torch.int64, device=values.device)
+    stride = values.stride(0) if values.numel() > 1 else 1
+    rc = load().hepf_histogram_values(values.data_ptr(), stride, values.shape[0], lo, hi, nbins, out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "hepf_histogram_values")
+    return out
 
 
 def reconstruct_tth(events: DeviceEvents, idx, n_idx: int, n_variations: int, seed: int, params: Params | None = None,

@@ -45,9 +45,51 @@ histogram_kernel(const hepf_best_t* __restrict__ best, int64_t n, int field, dou
     if (s_h[i]) atomicAdd(&out[i], (unsigned long long)s_h[i]);
 }
 
+// the same binning for a plain column of doubles (element k at values[k * stride]); every non-NaN value is filled
+__global__ void __launch_bounds__(H_THREADS)
+histogram_values_kernel(const double* __restrict__ values, int64_t stride_, int64_t n, double lo, double inv_w, int nbins,
+                        unsigned long long* __restrict__ out) {
+  extern __shared__ unsigned int s_h[];
+  for (int i = threadIdx.x; i < nbins + 2; i += H_THREADS) s_h[i] = 0u;
+  __syncthreads();
+  const int64_t stride = (int64_t)gridDim.x * H_THREADS;
+  for (int64_t k = (int64_t)blockIdx.x * H_THREADS + threadIdx.x; k < n; k += stride) {
+    const double t = __dmul_rn(__dadd_rn(__ldcs(values + k * stride_), -lo), inv_w);
+    if (t != t) continue;
+    const int bin = t < 0.0 ? 0 : (t >= (double)nbins ? nbins + 1 : 1 + (int)t);
+    atomicAdd(&s_h[bin], 1u);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < nbins + 2; i += H_THREADS)
+    if (s_h[i]) atomicAdd(&out[i], (unsigned long long)s_h[i]);
+}
+
 }  // namespace hepf
 
 using namespace hepf;
+
+extern "C" int hepf_histogram_values(const double* values, int64_t stride, int64_t n, double lo, double hi, int32_t nbins,
+                                     uint64_t* out, void* stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (n < 0 || stride < 1 || nbins < 1 || nbins > H_MAX_BINS || !(hi > lo)) {
+    set_error("hepf_histogram_values: need n >= 0, stride >= 1, 1 <= nbins <= %d and hi > lo", H_MAX_BINS); return HEPF_ERR_ARG;
+  }
+  if (!out || !aligned(out, 8) || (n > 0 && (!values || !aligned(values, 8)))) {
+    set_error("hepf_histogram_values: values/out NULL or misaligned"); return HEPF_ERR_ARG;
+  }
+  HEPF_CUDA_TRY(cudaMemsetAsync(out, 0, sizeof(uint64_t) * (size_t)(nbins + 2), stream));
+  if (n == 0) return HEPF_OK;
+  int dev = 0, sms = 148;
+  HEPF_CUDA_TRY(cudaGetDevice(&dev));
+  HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int64_t want = (n + H_THREADS - 1) / H_THREADS, cap = (int64_t)sms * 8;
+  histogram_values_kernel<<<(unsigned)(want < cap ? want : cap), H_THREADS, sizeof(unsigned int) * (size_t)(nbins + 2), stream>>>(
+      values, stride, n, lo, (double)nbins / (hi - lo), nbins, reinterpret_cast<unsigned long long*>(out));
+  count_launch();
+  HEPF_CUDA_TRY(cudaGetLastError());
+  return HEPF_OK;
+}
+
 
 extern "C" int hepf_histogram(const hepf_best_t* best, int64_t n, int field, double lo, double hi, int32_t nbins,
                               uint64_t* out, void* stream_) {

@@ -924,12 +924,56 @@ __device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_
 }
 
 // One thread per listed event (grid-stride: the grid is sized from the capacity, the length may live on the device).
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 4)   // 128 registers: the kernel is a chain of dependent FP64 operations, more resident warps hide it
 reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, const int64_t* __restrict__ n_dev, int64_t n_cap, uint32_t k0,
                      uint32_t k1, hepf_tth_params_t P, const uint2* __restrict__ winners, hepf_best_t* __restrict__ out) {
   const int64_t n_idx = list_length(n_dev, n_cap);
   for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_idx; k += (int64_t)gridDim.x * blockDim.x)
     finalize_event(ev, idx, k, k0, k1, P, winners, out);
+}
+
+// hepf_tth_system: invariant mass and transverse momentum of the reconstructed ttH system of each record (PAPER.md:410-442,
+// App. 8.2: "TLorentzVector ttH = Top + Tbar + Higgs; mTTH = ttH.M(); ptTTH = ttH.Pt();").  One thread per record: the
+// scales of the record's variation are drawn again (same Philox keys), the eight four-vectors l+, l-, nu, nubar, b, bbar,
+// h1, h2 are added in that order, every operation one IEEE operation in a fixed order (bit-identical to the definition).
+__global__ void __launch_bounds__(128)
+tth_system_kernel(RecoCols ev, const hepf_best_t* __restrict__ best, int64_t n, uint32_t k0, uint32_t k1, hepf_tth_params_t P,
+                  double2* __restrict__ out) {
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+    const hepf_best_t* b = best + k;
+    double2 r = make_double2(CUDART_NAN, CUDART_NAN);
+    const int64_t e = (int64_t)b->event - ev.out_off;
+    if ((b->status & 1u) && e >= 0 && e < ev.n) {
+      const EventHead h = load_head(ev, e);
+      const int slots[6] = {h.lp_slot, 1 - h.lp_slot, 2 + b->jet_b, 2 + b->jet_bbar, 2 + b->jet_h1, 2 + b->jet_h2};
+      const double nx = b->nu[0], ny = b->nu[1], nz = b->nu[2], qx = b->nubar[0], qy = b->nubar[1], qz = b->nubar[2];
+      const double en = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(nx, nx), __dmul_rn(ny, ny)), __dmul_rn(nz, nz)));
+      const double eq = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(qx, qx), __dmul_rn(qy, qy)), __dmul_rn(qz, qz)));
+      double sx = 0.0, sy = 0.0, sz = 0.0, se = 0.0;
+#pragma unroll 1
+      for (int i = 0; i < 8; i++) {        // order: l+, l-, nu, nubar, b, bbar, h1, h2
+        double px, py, pz, pe;
+        if (i == 2) { px = nx; py = ny; pz = nz; pe = en; }
+        else if (i == 3) { px = qx; py = qy; pz = qz; pe = eq; }
+        else {
+          const int t = slots[i < 2 ? i : i - 2];
+          double obj[4], ks; load_object(ev, e, t, P, obj, ks);
+          uint32_t x[4];
+          philox4x32_10((uint32_t)h.gidx, (uint32_t)(h.gidx >> 32), (uint32_t)b->variation, 0x54544800u + (t >> 1), k0, k1, x);
+          double z[2]; block_normals(x, z[0], z[1]);
+          const double sc = scale_of(ks, z[t & 1], P.s_min);
+          px = __dmul_rn(sc, obj[0]); py = __dmul_rn(sc, obj[1]); pz = __dmul_rn(sc, obj[2]); pe = __dmul_rn(sc, obj[3]);
+        }
+        if (i == 0) { sx = px; sy = py; sz = pz; se = pe; }
+        else { sx = __dadd_rn(sx, px); sy = __dadd_rn(sy, py); sz = __dadd_rn(sz, pz); se = __dadd_rn(se, pe); }
+      }
+      const double p2 = __dadd_rn(__dadd_rn(__dmul_rn(sx, sx), __dmul_rn(sy, sy)), __dmul_rn(sz, sz));
+      const double m2 = __dadd_rn(__dmul_rn(se, se), -p2);
+      r.x = __dsqrt_rn(m2 > 0.0 ? m2 : 0.0);
+      r.y = __dsqrt_rn(__dadd_rn(__dmul_rn(sx, sx), __dmul_rn(sy, sy)));
+    }
+    out[k] = r;
+  }
 }
 
 template <int VC, int NBT, int RW, int MINB>
@@ -1036,6 +1080,29 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, con
                                                                              (uint32_t)(seed >> 32), P, winners, out_best);
   count_launch();
   timing_mark(T_RECO3, stream);
+  HEPF_CUDA_TRY(cudaGetLastError());
+  return HEPF_OK;
+}
+
+extern "C" int hepf_tth_system(const hepf_events_t* events, const hepf_best_t* best, int64_t n, uint64_t seed,
+                               const hepf_tth_params_t* host_params, double* out, void* stream_) {
+  int rc = check_events(events);
+  if (rc != HEPF_OK) return rc;
+  if (n < 0) { set_error("hepf_tth_system: n < 0"); return HEPF_ERR_ARG; }
+  if (n == 0) return HEPF_OK;
+  if (!best || !aligned(best, 16) || !out || !aligned(out, 16)) { set_error("hepf_tth_system: best/out NULL or misaligned"); return HEPF_ERR_ARG; }
+  hepf_tth_params_t P;
+  if (host_params) P = *host_params; else hepf_default_params(&P);
+  const RecoCols cols{events->lep_px, events->lep_py, events->lep_pz, events->lep_e, events->jet_px, events->jet_py,
+                      events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags,
+                      events->n_events, events->stride, events->event_base, 0};
+  int dev = 0, sms = 148;
+  HEPF_CUDA_TRY(cudaGetDevice(&dev));
+  HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int64_t want = (n + 127) / 128, cap = (int64_t)sms * 16;
+  tth_system_kernel<<<(unsigned)(want < cap ? want : cap), 128, 0, (cudaStream_t)stream_>>>(
+      cols, best, n, (uint32_t)seed, (uint32_t)(seed >> 32), P, reinterpret_cast<double2*>(out));
+  count_launch();
   HEPF_CUDA_TRY(cudaGetLastError());
   return HEPF_OK;
 }

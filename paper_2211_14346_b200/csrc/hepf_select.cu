@@ -27,6 +27,8 @@ enum : uint32_t { NEED_LEP_PT = 1, NEED_LEP_ETA = 2, NEED_JET_PT = 4, NEED_JET_E
 struct CutChain {
   int n;
   uint32_t need;
+  int rec_cut;            // position of the recording cut (HEPF_CUT_MET_GT_RECORD), -1 = none
+  double rec_default;     // value of the derived column for events that do not pass it
   hepf_cut_t c[HEPF_MAX_CUTS];
 };
 
@@ -41,7 +43,7 @@ __device__ __forceinline__ double pick(const double2& v, int k) { return k ? v.y
 
 __global__ void __launch_bounds__(SEL_THREADS)
 select_eval_kernel(SelCols ev, CutChain chain, int64_t n_tiles, int64_t tiles_per_block, uint2* __restrict__ masks,
-                   uint32_t* __restrict__ block_count, unsigned long long* __restrict__ cutflow) {
+                   uint32_t* __restrict__ block_count, unsigned long long* __restrict__ cutflow, double* __restrict__ derived) {
   __shared__ unsigned int s_cf[HEPF_MAX_CUTS];
   __shared__ unsigned int s_count;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -95,7 +97,8 @@ select_eval_kernel(SelCols ev, CutChain chain, int64_t n_tiles, int64_t tiles_pe
                 cnt += (s < n_jet) && ((tagmask >> s) & 1u) && pick(jpt[s], k) > cut.lo && fabs(pick(jeta[s], k)) < cut.hi;
               ok = cnt >= (int)cut.n;
             } break;
-            case HEPF_CUT_MET_GT: ok = pick(met, k) > cut.lo; break;
+            case HEPF_CUT_MET_GT:
+            case HEPF_CUT_MET_GT_RECORD: ok = pick(met, k) > cut.lo; break;
             case HEPF_CUT_MLL_GT: ok = pick(mll, k) > cut.lo; break;
             case HEPF_CUT_MLL_OUTSIDE: ok = pick(mll, k) < cut.lo || pick(mll, k) > cut.hi; break;
             default: ok = false;
@@ -105,6 +108,15 @@ select_eval_kernel(SelCols ev, CutChain chain, int64_t n_tiles, int64_t tiles_pe
         }
         pass[k] = alive;
         fail_at[k] = passed;
+      }
+      // the recording cut's side effect ("ETmis = met_met; ETmis *= 1.05"): one rounded multiplication
+      // for the events that passed the chain up to and including it, the default value for all others
+      if (derived) {
+        const double sc = chain.c[chain.rec_cut].hi;
+        const double d0 = fail_at[0] > chain.rec_cut ? __dmul_rn(met.x, sc) : chain.rec_default;
+        const double d1 = fail_at[1] > chain.rec_cut ? __dmul_rn(met.y, sc) : chain.rec_default;
+        if (i0 + 1 < ev.n) __stcs(reinterpret_cast<double2*>(derived + i0), make_double2(d0, d1));
+        else derived[i0] = d0;
       }
     }
     // ---- warp compaction: survivor masks (even events, odd events) ---------------------------------------------
@@ -194,9 +206,9 @@ extern "C" size_t hepf_select_workspace_bytes(int64_t n_events) {
   return align_up((size_t)(n_tiles + 1) * SEL_WARPS * sizeof(uint2), 256) + 4096 * sizeof(uint32_t);
 }
 
-extern "C" int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
-                           int64_t* out_count, int64_t* out_cutflow, void* ws, size_t ws_bytes, void* stream_) {
-  cudaStream_t stream = (cudaStream_t)stream_;
+static int select_impl(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
+                       int64_t* out_count, int64_t* out_cutflow, double* out_derived, double derived_default, void* ws,
+                       size_t ws_bytes, cudaStream_t stream) {
   int rc = check_events(events);
   if (rc != HEPF_OK) return rc;
   if (n_cuts < 0 || n_cuts > HEPF_MAX_CUTS || (n_cuts > 0 && !host_cuts)) {
@@ -213,9 +225,13 @@ extern "C" int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_c
   }
   CutChain chain{};
   chain.n = n_cuts;
+  chain.rec_cut = -1; chain.rec_default = derived_default;
   for (int c = 0; c < n_cuts; c++) {
     chain.c[c] = host_cuts[c];
     switch (host_cuts[c].kind) {
+      case HEPF_CUT_MET_GT_RECORD:
+        if (chain.rec_cut >= 0) { set_error("hepf_select: at most one recording cut per chain"); return HEPF_ERR_ARG; }
+        chain.rec_cut = c; chain.need |= NEED_MET; break;
       case HEPF_CUT_LEP_PT_GT: chain.need |= NEED_LEP_PT; break;
       case HEPF_CUT_LEP_ABSETA_LT: chain.need |= NEED_LEP_ETA; break;
       case HEPF_CUT_NJET_GE: case HEPF_CUT_NBJET_GE: chain.need |= NEED_JET_PT | NEED_JET_ETA; break;
@@ -224,6 +240,9 @@ extern "C" int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_c
       case HEPF_CUT_NLEP_EQ: case HEPF_CUT_LEP_OS: break;
       default: set_error("hepf_select: unknown cut kind %u at position %d", host_cuts[c].kind, c); return HEPF_ERR_ARG;
     }
+  }
+  if (out_derived && (chain.rec_cut < 0 || !aligned(out_derived, 16))) {
+    set_error("hepf_select_record: out_derived needs a HEPF_CUT_MET_GT_RECORD cut in the chain and 16-byte alignment"); return HEPF_ERR_ARG;
   }
   if (out_cutflow && n_cuts > 0) HEPF_CUDA_TRY(cudaMemsetAsync(out_cutflow, 0, sizeof(int64_t) * n_cuts, stream));
   if (n == 0) { HEPF_CUDA_TRY(cudaMemsetAsync(out_count, 0, sizeof(int64_t), stream)); return HEPF_OK; }
@@ -245,7 +264,8 @@ extern "C" int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_c
                events->flags, n, events->stride};
   timing_mark(T_SEL0, stream);
   select_eval_kernel<<<grid, SEL_THREADS, 0, stream>>>(cols, chain, n_tiles, tpb, masks, block_count,
-                                                       (n_cuts > 0) ? reinterpret_cast<unsigned long long*>(out_cutflow) : nullptr);
+                                                       (n_cuts > 0) ? reinterpret_cast<unsigned long long*>(out_cutflow) : nullptr,
+                                                       out_derived);
   count_launch();
   HEPF_CUDA_TRY(cudaGetLastError());
   timing_mark(T_SEL1, stream);
@@ -254,4 +274,17 @@ extern "C" int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_c
   timing_mark(T_SEL2, stream);
   HEPF_CUDA_TRY(cudaGetLastError());
   return HEPF_OK;
+}
+
+extern "C" int hepf_select(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
+                           int64_t* out_count, int64_t* out_cutflow, void* ws, size_t ws_bytes, void* stream_) {
+  return select_impl(events, host_cuts, n_cuts, out_idx, out_count, out_cutflow, nullptr, 0.0, ws, ws_bytes, (cudaStream_t)stream_);
+}
+
+extern "C" int hepf_select_record(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
+                                  int64_t* out_count, int64_t* out_cutflow, double* out_derived, double derived_default,
+                                  void* ws, size_t ws_bytes, void* stream_) {
+  if (!out_derived) { set_error("hepf_select_record: out_derived is NULL"); return HEPF_ERR_ARG; }
+  return select_impl(events, host_cuts, n_cuts, out_idx, out_count, out_cutflow, out_derived, derived_default, ws, ws_bytes,
+                     (cudaStream_t)stream_);
 }

@@ -153,6 +153,19 @@ def test_variation_counts_and_lane_mappings(hepf, V):
     assert_parity(st, got, want, aux, V, 1234 + V, label=f"V={V}")
 
 
+def test_paper_scale_variation_counts(hepf):
+    """the paper's ttH_sci (1024 pseudo-experiments per event) and ttH_scinp (128,
+    PAPER.md:146) run through the same kernels; 64 chunks of 16 variations per event.  All selected events of a 1500-event
+    sample at V = 1024 and V = 128 against the oracle."""
+    st = hs.CONFIGS[2].events(1500)
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, hs.CHAIN_BASE)
+    for V in (1024, 128):
+        got = _gpu_reco(hepf, dev, idx_t, n, V, 0x5C1 + V)
+        want, aux = oracle.reconstruct_tth(st, idx, V, 0x5C1 + V, n_threads=16)
+        cls = assert_parity(st, got, want, aux, V, 0x5C1 + V, max_oracle_far_frac=2e-2, label=f"ttH_sci V={V}")
+        assert cls["match"] > 0.97 * n and (got["variation"] >= 64).any()
+
+
 def test_six_b_candidates_parity(hepf):
     cfg = hs.CONFIGS[3]
     st = cfg.events(3000)
@@ -560,3 +573,61 @@ def test_garbage_inputs_terminate_and_keep_the_status_contract(hepf):
     assert (c["status"] == 2).all()                                      # dileptonic sample: not applicable
     h = hepf.histogram(hepf.reconstruct_tth(dev, idx_t, n, 8, 5), n, "loglik", -50.0, 10.0, 32).cpu().numpy()
     assert 0 < int(h.sum()) <= int(solved.sum())
+
+
+# ------------------------------------------------------------------------ derived per-event variables
+@pytest.mark.parametrize("n", [1, 2, 3, 511, 513, 100_001])
+def test_recording_cut_bit_exact(hepf, n):
+    """hepf_select_record (the cut that writes ETmis = 1.05 met) against the oracle: survivor list, cutflow
+    and the derived column bit for bit, at ragged sizes (odd n: the last event is a scalar store)."""
+    import torch
+    st = hs.generate(max(n, 2), 31 + n, bkg_frac=0.3, with_truth=False)
+    st.n_events = n
+    chain = hs.CHAIN_TIGHT8[:6] + [(10, 0, 55.0, 1.05)] + hs.CHAIN_TIGHT8[7:]
+    dev = hepf.DeviceEvents.from_host(st)
+    idx_t, count, cf, derived = hepf.select_record(dev, chain, derived_default=-3.5)
+    torch.cuda.synchronize()
+    want_idx, want_cf, want_d = oracle.select_record(st, chain, derived_default=-3.5)
+    m = int(count.item())
+    assert m == len(want_idx) and np.array_equal(idx_t[:m].cpu().numpy().view(np.uint32), want_idx)
+    assert np.array_equal(cf.cpu().numpy(), want_cf)
+    assert derived.cpu().numpy().tobytes() == want_d.tobytes()
+    # in plain hepf_select the same cut kind only filters
+    i2, c2, cf2 = hepf.select(dev, chain)
+    torch.cuda.synchronize()
+    assert int(c2.item()) == m and np.array_equal(cf2.cpu().numpy(), want_cf)
+
+
+def test_tth_system_and_value_histograms(hepf):
+    """hepf_tth_system (m_ttH, pT_ttH of PAPER.md:410-442): (a) fed with the ORACLE's records it must reproduce the oracle's
+    values bit for bit (same operation sequence); (b) on its own records it agrees to 1e-9 wherever the records do;
+    hepf_histogram_values of the derived columns is bit-exact."""
+    import torch
+    from paper_2211_14346_b200.binding import best_to_numpy
+    cfg = hs.CONFIGS[1]
+    st = cfg.events(6000)
+    dev, idx_t, n, idx, _ = _gpu_select(hepf, st, cfg.cuts)
+    want, aux = oracle.reconstruct_tth(st, idx, cfg.n_variations, cfg.reco_seed, n_threads=8)
+    want_sys = oracle.tth_system(st, want, cfg.reco_seed)
+    orc_rec = torch.from_numpy(want.view(np.uint8).reshape(-1, 128).copy()).cuda()
+    got_sys = hepf.tth_system(dev, orc_rec, n, cfg.reco_seed).cpu().numpy()
+    nan = np.isnan(want_sys)
+    assert np.array_equal(np.isnan(got_sys), nan) and got_sys[~nan].tobytes() == want_sys[~nan].tobytes()   # (the NaN payloads differ in sign)
+    rec_t = hepf.reconstruct_tth(dev, idx_t, n, cfg.n_variations, cfg.reco_seed)
+    own = hepf.tth_system(dev, rec_t, n, cfg.reco_seed)
+    torch.cuda.synchronize()
+    rec = best_to_numpy(rec_t)
+    same = ((rec["status"] & 1) == 1) & ((want["status"] & 1) == 1) & (rec["variation"] == want["variation"]) & (rec["root"] == want["root"]) \
+        & (np.abs(rec["nu"] - want["nu"]).max(axis=1) <= 1e-9 * np.maximum(1.0, np.abs(want["nu"]).max(axis=1)))
+    o = own.cpu().numpy()
+    assert same.sum() > 0.95 * n and np.allclose(o[same], want_sys[same], rtol=1e-9, atol=0)
+    assert np.isnan(o[(rec["status"] & 1) == 0]).all()
+    for col, lo, hi, nb in ((0, 300.0, 2000.0, 170), (1, 0.0, 400.0, 64)):
+        h = hepf.histogram_values(own[:, col], lo, hi, nb).cpu().numpy().astype(np.uint64)
+        assert np.array_equal(h, oracle.histogram_values(o[:, col], lo, hi, nb))
+        assert int(h.sum()) == int((rec["status"] & 1).sum())
+    # the ETmis column of a recording cut through the same histogram
+    chain = [(10, 0, 30.0, 1.05)]
+    _, _, _, derived = hepf.select_record(dev, chain, derived_default=float("nan"))
+    hd = hepf.histogram_values(derived, 0.0, 500.0, 100).cpu().numpy().astype(np.uint64)
+    assert np.array_equal(hd, oracle.histogram_values(oracle.select_record(st, chain, float("nan"))[2], 0.0, 500.0, 100))
