@@ -352,6 +352,34 @@ class TthRun:
                   "eval+scatter_ms": km["select"]}
         return roof, select
 
+    def planned_select(self, reps=20):
+        """measured filter ratios -> hepf_plan_chain -> hepf_select_planned, timed against hepf_select."""
+        import torch
+        h = self.hepf
+        stats = h.cut_stats(self.dev, self.cfg.cuts, 16).cpu().numpy()
+        p = stats[:-1] / max(1, stats[-1])
+        order, split, planned_b, one_b = h.plan_chain(self.cfg.cuts, p)
+        ws = torch.empty(int(h.load().hepf_select_planned_workspace_bytes(self.n)) + 256, dtype=torch.uint8, device="cuda")
+        idx2 = torch.empty_like(self.out_idx); cnt2 = torch.zeros_like(self.out_count)
+
+        def timed(f):
+            for _ in range(3):
+                f()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(self.stream)
+            for _ in range(reps):
+                f()
+            e1.record(self.stream)
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / reps
+        ms_one = timed(lambda: h.select(self.dev, self.cfg.cuts, with_cutflow=False, out_idx=self.out_idx, out_count=self.out_count, ws=self.ws, stream=self.stream))
+        ms_two = timed(lambda: h.select_planned(self.dev, self.cfg.cuts, order, split, out_idx=idx2, out_count=cnt2, ws=ws, stream=self.stream))
+        same = bool(int(cnt2.item()) == int(self.out_count.item()) and torch.equal(idx2[:int(cnt2.item())], self.out_idx[:int(cnt2.item())]))
+        return {"measured_pass_fractions": [float(x) for x in p], "order": order, "split": split,
+                "model_bytes_per_event": {"planned": planned_b, "one_phase": one_b},
+                "ms_hepf_select_no_cutflow": ms_one, "ms_hepf_select_planned": ms_two, "same_survivors": same,
+                "note": "phase 1 (cuts order[:split]) over every event, phase 2 over phase 1's survivors only; PAPER.md:192-198"}
+
     def free(self):
         import torch
         for a in ("dev", "out_idx", "out_best", "ws", "reco_ws", "store"):
@@ -470,6 +498,8 @@ def main():
                              else f"inputs ({516 * n / 1e6:.1f} MB) fit in L2: parity-test configuration, not a bench line"),
                       "parallelism": f"dp{world} (events sharded by global index, no collective)"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": run.launches, "roofline": roofline, "select": select_line}
+    if args.workload == "cfg4" and world == 1:
+        out["planned_select"] = run.planned_select()
     idx_host = run.idx_host
     if not args.no_cpu_baseline and world == 1:      # the oracle is timed beside the GPU number on rank 0 at N = 1 only
         cores = os.cpu_count() or 1
@@ -488,6 +518,8 @@ def main():
             roof, sel = r.rooflines(ms, sm_max, sms, prof)
             extra[f"cfg{cid}"] = {"workload": c.name, "ms_per_step": ms, "steps": k, "value": r.n_solves / (ms * 1e-3), "unit": UNIT,
                                   "selected": r.n_sel, "solves_per_step": r.n_solves, "roofline": roof, "select": sel}
+            if cid == 4:
+                extra["cfg4"]["planned_select"] = r.planned_select()
             r.free()
         free, _ = torch.cuda.mem_get_info()
         n5 = hs.PHILOX_CFG5["n"]

@@ -119,6 +119,36 @@ int hepf_select_record(const hepf_events_t* events, const hepf_cut_t* host_cuts,
                        size_t ws_bytes, void* stream);
 
 /*
+ * The device analogue of the paper's cut-level scheduler (section 5.2: "HEP-Frame dynamically optimises
+ * the ordering of the cuts during execution", from each cut's measured filter ratio and execution time, "respecting the
+ * dependencies among cuts").  On the GPU a cut's cost is the bytes of the columns it reads, and the lever is not the order of
+ * the compares but WHICH EVENTS' columns are fetched at all: a chain is split into two phases, phase 1 (cheap columns) over
+ * every event, phase 2 (the rest) over phase 1's survivors only.
+ *   hepf_cut_stats      measures: every cut on its own on the events of every `sample_every`-th tile of 512 events;
+ *                       out_pass device int64[n_cuts + 1]: [c] = events that pass cut c, [n_cuts] = events looked at.
+ *   hepf_plan_chain     decides (host only, no device): given the measured pass fractions and a dependency mask (bit k of
+ *                       dep_mask[c] set = cut c must not run in an earlier phase than cut k; NULL = cuts commute), the phase-1 set
+ *                       that minimises the expected bytes read per event,
+ *                         4 + B(phase 1) + (1 - (1 - p1)^8) (4 + B(phase 2)) / 0.55 + 8 p1,   p1 = product of phase 1's pass fractions,
+ *                       B = bytes of the column groups named.  Phase 2 gathers: it moves whole 64-byte DRAM atoms (eight events of
+ *                       a column; fetched if any of them survives) at about 55 % of the streaming bandwidth (measured on B200).
+ *                       One phase is kept unless two save at least 10 %.  out_order: a permutation of the cuts,
+ *                       phase 1 first, user order inside a phase; out_split: cuts [0, split) of it form phase 1 (n_cuts = one
+ *                       phase); out_bytes_per_event (or NULL): [0] planned, [1] one phase.
+ *   hepf_select_planned executes a chain in that order with that split.  The survivor list is that of hepf_select (cuts are
+ *                       pure predicates: the set does not depend on the order; the list stays ascending).  out_cutflow, if
+ *                       given, is in EXECUTED order: [k] = events that passed the first k + 1 executed cuts.  A recording
+ *                       cut cannot be planned.  ws >= hepf_select_planned_workspace_bytes(n_events), 256-byte aligned.
+ */
+int hepf_cut_stats(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, int64_t sample_every,
+                   int64_t* out_pass, void* stream);
+int hepf_plan_chain(const hepf_cut_t* host_cuts, int n_cuts, const double* pass_frac, const uint32_t* dep_mask, int* out_order,
+                    int* out_split, double* out_bytes_per_event);
+int hepf_select_planned(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, const int* order, int split,
+                        uint32_t* out_idx, int64_t* out_count, int64_t* out_cutflow, void* ws, size_t ws_bytes, void* stream);
+size_t hepf_select_planned_workspace_bytes(int64_t n_events);
+
+/*
  * hepf_reconstruct_tth — for each listed event: for every smearing variation v < n_variations draw ten
  * standard normals from Philox4x32-10 keyed (seed; event_base+e, v, block) + Box-Muller, scale the two leptons
  * and the jets, propagate the change to the missing transverse momentum, and for every ordered pair of b-jet

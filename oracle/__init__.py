@@ -74,6 +74,7 @@ def lib():
         L.orc_select_record.argtypes = [C.POINTER(Events), C.POINTER(Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]
         L.orc_tth_system.argtypes = [C.POINTER(Events), C.c_void_p, C.c_int64, C.c_uint64, C.POINTER(Params), C.c_void_p]
         L.orc_histogram_values.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_int32, C.c_void_p]
+        L.orc_cut_stats.argtypes = [C.POINTER(Events), C.POINTER(Cut), C.c_int, C.c_int64, C.c_void_p]
         L.orc_reconstruct_tth.argtypes = [C.POINTER(Events), C.c_void_p, C.c_int64, C.c_int32, C.c_uint64,
                                           C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_int]
         L.orc_solve_pairing.argtypes = [C.c_void_p] * 6 + [C.c_int, C.POINTER(Params), C.POINTER(Pairing)]
@@ -163,6 +164,16 @@ def select_record(store, chain, derived_default: float = 0.0):
     if rc != 0:
         raise RuntimeError(f"orc_select_record: {rc}")
     return idx[: int(count[0])].copy(), cutflow[: len(chain)].copy(), derived
+
+
+def cut_stats(store, chain, sample_every: int = 1) -> np.ndarray:
+    """int64[n_cuts + 1]: events of the sample passing each cut on its own, and the sample size."""
+    ev = events_view(store)
+    out = np.zeros(len(chain) + 1, dtype=np.int64)
+    rc = lib().orc_cut_stats(C.byref(ev), make_cuts(chain), len(chain), sample_every, out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_cut_stats: {rc}")
+    return out
 
 
 def tth_system(store, best, seed: int, params: Params | None = None) -> np.ndarray:

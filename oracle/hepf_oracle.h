@@ -93,6 +93,8 @@ int orc_select(const orc_events_t* ev, const orc_cut_t* cuts, int n_cuts, uint32
 /* a chain with a recording cut (ORC_MET_GT_RECORD): see oracle_select.cpp */
 int orc_select_record(const orc_events_t* ev, const orc_cut_t* cuts, int n_cuts, uint32_t* out_idx, int64_t* out_count,
                       int64_t* out_cutflow, double* out_derived, double derived_default);
+/* per-cut filter ratios on a sample (oracle_select.cpp) */
+int orc_cut_stats(const orc_events_t* ev, const orc_cut_t* cuts, int n_cuts, int64_t sample_every, int64_t* out_pass);
 /* O4: n_threads > 1 only distributes whole events over OpenMP threads; per-event arithmetic is unchanged */
 int orc_reconstruct_tth(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
                         uint64_t seed, const orc_params_t* params, orc_best_t* out_best, orc_aux_t* out_aux,

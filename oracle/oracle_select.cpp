@@ -79,3 +79,17 @@ extern "C" int orc_select_record(const orc_events_t* ev, const orc_cut_t* cuts, 
   if (out_count) *out_count = n;
   return 0;
 }
+
+// PAPER.md:194-196 (§5.2): the framework measures each cut's filter ratio (and execution time) to order the pipeline.  The
+// filter ratio of a cut ON ITS OWN: out_pass[c] = events of the sample that pass cut c alone, out_pass[n_cuts] = sample size.
+// The sample is every `sample_every`-th block of 512 consecutive events (blocks 0, sample_every, 2 sample_every, ...).
+extern "C" int orc_cut_stats(const orc_events_t* ev, const orc_cut_t* cuts, int n_cuts, int64_t sample_every, int64_t* out_pass) {
+  if (!ev || n_cuts < 0 || n_cuts > 32 || (n_cuts > 0 && !cuts) || sample_every < 1 || !out_pass) return -1;
+  for (int c = 0; c <= n_cuts; c++) out_pass[c] = 0;
+  for (int64_t i = 0; i < ev->n_events; i++) {
+    if ((i / 512) % sample_every != 0) continue;
+    out_pass[n_cuts]++;
+    for (int c = 0; c < n_cuts; c++) if (pass_cut(ev, i, cuts[c])) out_pass[c]++;
+  }
+  return 0;
+}

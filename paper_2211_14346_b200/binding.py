@@ -84,6 +84,12 @@ def load():
                                          C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
         L.hepf_tth_system.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_uint64, C.POINTER(Params), C.c_void_p, C.c_void_p]
         L.hepf_histogram_values.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
+        L.hepf_cut_stats.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_int64, C.c_void_p, C.c_void_p]
+        L.hepf_plan_chain.argtypes = [C.POINTER(_Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int), C.c_void_p]
+        L.hepf_select_planned.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
+                                          C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hepf_select_planned_workspace_bytes.restype = C.c_size_t
+        L.hepf_select_planned_workspace_bytes.argtypes = [C.c_int64]
         L.hepf_timing_enable.argtypes = [C.c_int]
         L.hepf_timing_ms.restype = C.c_double
         L.hepf_timing_ms.argtypes = [C.c_int, C.c_int]
@@ -235,6 +241,50 @@ def histogram_values(values, lo: float, hi: float, nbins: int, *, out=None, stre
     rc = load().hepf_histogram_values(values.data_ptr(), stride, values.shape[0], lo, hi, nbins, out.data_ptr(), _stream_ptr(stream))
     _check(rc, "hepf_histogram_values")
     return out
+
+
+def cut_stats(events: DeviceEvents, chain, sample_every: int = 1, *, stream=None):
+    """hepf_cut_stats: int64 device tensor [n_cuts + 1]: per-cut pass counts (each cut on its own) and the number of events looked at."""
+    import torch
+    out = torch.zeros(len(chain) + 1, dtype=torch.int64, device=events.cols.device)
+    ev = events.view()
+    rc = load().hepf_cut_stats(C.byref(ev), make_cuts(chain), len(chain), sample_every, out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "hepf_cut_stats")
+    return out
+
+
+def plan_chain(chain, pass_frac, dep_mask=None):
+    """hepf_plan_chain (host only): (order, split, planned bytes/event, one-phase bytes/event)."""
+    n = len(chain)
+    pf = np.ascontiguousarray(pass_frac, dtype=np.float64)
+    dm = np.ascontiguousarray(dep_mask, dtype=np.uint32) if dep_mask is not None else None
+    order = np.zeros(max(n, 1), dtype=np.int32); split = C.c_int(0); by = np.zeros(2)
+    rc = load().hepf_plan_chain(make_cuts(chain), n, pf.ctypes.data, dm.ctypes.data if dm is not None else None, order.ctypes.data,
+                                C.byref(split), by.ctypes.data)
+    _check(rc, "hepf_plan_chain")
+    return [int(x) for x in order[:n]], int(split.value), float(by[0]), float(by[1])
+
+
+def select_planned(events: DeviceEvents, chain, order, split: int, *, with_cutflow: bool = False, out_idx=None, out_count=None, ws=None, stream=None):
+    """hepf_select_planned: (out_idx, out_count, cutflow in executed order or None)."""
+    import torch
+    L = load()
+    dev = events.cols.device
+    n = events.n_events
+    if out_idx is None:
+        out_idx = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    if out_count is None:
+        out_count = torch.zeros(1, dtype=torch.int64, device=dev)
+    cf = torch.zeros(max(len(chain), 1), dtype=torch.int64, device=dev) if with_cutflow else None
+    need = L.hepf_select_planned_workspace_bytes(n)
+    if ws is None or ws.numel() < need:
+        ws = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    ev = events.view()
+    od = np.ascontiguousarray(order, dtype=np.int32)
+    rc = L.hepf_select_planned(C.byref(ev), make_cuts(chain), len(chain), od.ctypes.data, split, out_idx.data_ptr(), out_count.data_ptr(),
+                               cf.data_ptr() if with_cutflow else None, ws.data_ptr(), ws.numel(), _stream_ptr(stream))
+    _check(rc, "hepf_select_planned")
+    return out_idx, out_count, (cf[: len(chain)] if with_cutflow else None)
 
 
 def reconstruct_tth(events: DeviceEvents, idx, n_idx: int, n_variations: int, seed: int, params: Params | None = None,

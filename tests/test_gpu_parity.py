@@ -631,3 +631,34 @@ def test_tth_system_and_value_histograms(hepf):
     _, _, _, derived = hepf.select_record(dev, chain, derived_default=float("nan"))
     hd = hepf.histogram_values(derived, 0.0, 500.0, 100).cpu().numpy().astype(np.uint64)
     assert np.array_equal(hd, oracle.histogram_values(oracle.select_record(st, chain, float("nan"))[2], 0.0, 500.0, 100))
+
+
+# ------------------------------------------------------------------------ cut-level scheduler analogue
+def test_cut_stats_and_planned_two_phase_select(hepf):
+    """hepf_cut_stats bit-exact against the oracle; hepf_plan_chain's plan executed by hepf_select_planned gives exactly
+    hepf_select's (= the oracle's) survivor list, whatever the order and the split; its cutflow is the oracle's for the
+    executed order."""
+    import torch
+    cfg = hs.CONFIGS[4]
+    for n in (1, 700, 250_001):
+        st = cfg.events(max(n, 2)); st.n_events = n
+        dev = hepf.DeviceEvents.from_host(st)
+        for every in (1, 7):
+            got = hepf.cut_stats(dev, cfg.cuts, every).cpu().numpy()
+            assert np.array_equal(got, oracle.cut_stats(st, cfg.cuts, every))
+        stats = hepf.cut_stats(dev, cfg.cuts, 1).cpu().numpy()
+        p = stats[:-1] / max(1, stats[-1])
+        order, split, planned, one = hepf.plan_chain(cfg.cuts, p)
+        want_idx, _ = oracle.select(st, cfg.cuts)
+        plans = [(order, split), (list(range(8)), 3), ([7, 6, 5, 4, 3, 2, 1, 0], 2), (list(range(8)), 8), ([4, 5, 0, 1, 2, 3, 6, 7], 2)]
+        for od, sp in plans:
+            idx_t, count, cf = hepf.select_planned(dev, cfg.cuts, od, sp, with_cutflow=True)
+            torch.cuda.synchronize()
+            m = int(count.item())
+            assert m == len(want_idx) and np.array_equal(idx_t[:m].cpu().numpy().view(np.uint32), want_idx), (n, od, sp)
+            _, want_cf = oracle.select(st, [cfg.cuts[c] for c in od])
+            assert np.array_equal(cf.cpu().numpy(), want_cf), (n, od, sp)
+    with pytest.raises(hepf.HepfError):
+        hepf.select_planned(dev, cfg.cuts, [0, 1, 2, 3, 4, 5, 6, 6], 4)
+    with pytest.raises(hepf.HepfError):
+        hepf.plan_chain([(10, 0, 30.0, 1.05)], [0.5])
