@@ -353,12 +353,10 @@ class TthRun:
         return roof, select
 
     def planned_select(self, reps=20):
-        """measured filter ratios -> hepf_plan_chain -> hepf_select_planned, timed against hepf_select."""
+        """measured filter ratios -> hepf_plan_chain -> hepf_select_planned, timed against hepf_select; the
+        same for a variant of the chain whose lepton-pT cut is tight enough for two phases to pay, and a forced split."""
         import torch
         h = self.hepf
-        stats = h.cut_stats(self.dev, self.cfg.cuts, 16).cpu().numpy()
-        p = stats[:-1] / max(1, stats[-1])
-        order, split, planned_b, one_b = h.plan_chain(self.cfg.cuts, p)
         ws = torch.empty(int(h.load().hepf_select_planned_workspace_bytes(self.n)) + 256, dtype=torch.uint8, device="cuda")
         idx2 = torch.empty_like(self.out_idx); cnt2 = torch.zeros_like(self.out_count)
 
@@ -372,13 +370,30 @@ class TthRun:
             e1.record(self.stream)
             torch.cuda.synchronize()
             return e0.elapsed_time(e1) / reps
-        ms_one = timed(lambda: h.select(self.dev, self.cfg.cuts, with_cutflow=False, out_idx=self.out_idx, out_count=self.out_count, ws=self.ws, stream=self.stream))
-        ms_two = timed(lambda: h.select_planned(self.dev, self.cfg.cuts, order, split, out_idx=idx2, out_count=cnt2, ws=ws, stream=self.stream))
-        same = bool(int(cnt2.item()) == int(self.out_count.item()) and torch.equal(idx2[:int(cnt2.item())], self.out_idx[:int(cnt2.item())]))
-        return {"measured_pass_fractions": [float(x) for x in p], "order": order, "split": split,
-                "model_bytes_per_event": {"planned": planned_b, "one_phase": one_b},
-                "ms_hepf_select_no_cutflow": ms_one, "ms_hepf_select_planned": ms_two, "same_survivors": same,
-                "note": "phase 1 (cuts order[:split]) over every event, phase 2 over phase 1's survivors only; PAPER.md:192-198"}
+
+        def one_chain(chain, force=None):
+            stats = h.cut_stats(self.dev, chain, 16).cpu().numpy()
+            p = stats[:-1] / max(1, stats[-1])
+            order, split, planned_b, one_b = h.plan_chain(chain, p)
+            if force:
+                order, split = force
+            ms_one = timed(lambda: h.select(self.dev, chain, with_cutflow=False, out_idx=self.out_idx, out_count=self.out_count, ws=self.ws, stream=self.stream))
+            ms_two = timed(lambda: h.select_planned(self.dev, chain, order, split, out_idx=idx2, out_count=cnt2, ws=ws, stream=self.stream))
+            m = int(cnt2.item())
+            same = bool(m == int(self.out_count.item()) and torch.equal(idx2[:m], self.out_idx[:m]))
+            return {"measured_pass_fractions": [round(float(x), 4) for x in p], "order": order, "split": split, "phases": 1 if split == len(chain) else 2,
+                    "model_bytes_per_event": {"planned": planned_b, "one_phase": one_b}, "survivors": m,
+                    "ms_hepf_select_no_cutflow": ms_one, "ms_hepf_select_planned": ms_two, "same_survivors": same}
+        chain = list(self.cfg.cuts)
+        out = {"planned": one_chain(chain), "note": "phase 1 (cuts order[:split]) over every event, phase 2 over phase 1's survivors only; PAPER.md:192-198"}
+        jets = [c for c, cut in enumerate(chain) if cut[0] in (hs.NJET_GE, hs.NBJET_GE)]
+        if jets and len(jets) < len(chain):
+            rest = [c for c in range(len(chain)) if c not in jets]
+            out["forced_jets_in_phase_2"] = one_chain(chain, force=(rest + jets, len(rest)))
+        tight = [(k, n, 90.0, hi) if k == hs.LEP_PT_GT else (k, n, lo, hi) for (k, n, lo, hi) in chain]
+        if tight != chain:
+            out["tight_lepton_pt_90_variant"] = one_chain(tight)
+        return out
 
     def free(self):
         import torch

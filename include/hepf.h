@@ -129,7 +129,8 @@ int hepf_select_record(const hepf_events_t* events, const hepf_cut_t* host_cuts,
  *   hepf_plan_chain     decides (host only, no device): given the measured pass fractions and a dependency mask (bit k of
  *                       dep_mask[c] set = cut c must not run in an earlier phase than cut k; NULL = cuts commute), the phase-1 set
  *                       that minimises the expected bytes read per event,
- *                         4 + B(phase 1) + (1 - (1 - p1)^8) (4 + B(phase 2)) / 0.55 + 8 p1,   p1 = product of phase 1's pass fractions,
+ *                         4 + B(phase 1) + (1 - (1 - p1)^8) (4 + B(phase 2)) / 0.55 + 8 p1,   p1 = product over phase 1's cut families (cuts
+ *                       reading the same columns count once, with their smallest pass fraction) of the pass fractions,
  *                       B = bytes of the column groups named.  Phase 2 gathers: it moves whole 64-byte DRAM atoms (eight events of
  *                       a column; fetched if any of them survives) at about 55 % of the streaming bandwidth (measured on B200).
  *                       One phase is kept unless two save at least 10 %.  out_order: a permutation of the cuts,

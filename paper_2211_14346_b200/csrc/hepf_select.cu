@@ -522,8 +522,19 @@ extern "C" int hepf_plan_chain(const hepf_cut_t* host_cuts, int n_cuts, const do
         if ((S1 >> c & 1u) && dep_mask && (dep_mask[c] & full & ~S1)) { S1 &= ~(1u << c); changed = true; }
     }
     if (S1 == 0 || S1 == full) continue;
-    uint32_t n1 = 0, n2 = 0; double p1 = 1.0;
-    for (int c = 0; c < n_cuts; c++) { if (S1 >> c & 1u) { n1 |= need[c]; p1 *= pass_frac[c]; } else n2 |= need[c]; }
+    // pass fraction of phase 1: cuts that read the same columns are strongly correlated (two jet-count thresholds on the same
+    // jets), so each such family counts once, with its SMALLEST pass fraction (an upper bound of the family's joint
+    // fraction); different families are taken as independent
+    uint32_t n1 = 0, n2 = 0, done = 0; double p1 = 1.0;
+    for (int c = 0; c < n_cuts; c++) {
+      if (!(S1 >> c & 1u)) { n2 |= need[c]; continue; }
+      n1 |= need[c];
+      if (done >> c & 1u) continue;
+      double pm = pass_frac[c];
+      for (int d = c + 1; d < n_cuts; d++)
+        if ((S1 >> d & 1u) && need[d] == need[c]) { done |= 1u << d; if (pass_frac[d] < pm) pm = pass_frac[d]; }
+      p1 *= pm;
+    }
     const double cost = two_phase_bytes(n1, n2, p1);
     if (cost < best) { best = cost; best_set = S1; }
   }

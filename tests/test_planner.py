@@ -27,7 +27,11 @@ def _brute(chain, p, dep):
         s1 = [c for c in range(n) if mask >> c & 1]
         if dep is not None and any((int(dep[c]) & ~mask & 0xffffffff) for c in s1):
             continue
-        p1 = float(np.prod([p[c] for c in s1]))
+        fam = {}
+        for c in s1:
+            key = frozenset(GROUP[chain[c][0]])
+            fam[key] = min(fam.get(key, 1.0), p[c])          # cuts on the same columns: one family, its smallest pass fraction
+        p1 = float(np.prod(list(fam.values())))
         cost = 4 + _bytes([chain[c] for c in s1]) + (1 - (1 - p1) ** 8) * (4 + _bytes([chain[c] for c in range(n) if not mask >> c & 1])) / 0.55 + 8 * p1
         best = min(best, cost)
     return (best if best < 0.9 * one else one), one
