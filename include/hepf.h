@@ -226,6 +226,20 @@ typedef struct {
 } hepf_chi2_t;   /* 80 bytes */
 int hepf_chi2_semilep(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, const hepf_chi2_params_t* host_params,
                       hepf_chi2_t* out, void* stream);
+/*
+ * hepf_chi2_single_top — the single-top variants of eq. (1) ("in single top quark events from Wt associated
+ * production, only 1 top quark and 2 W-bosons should be reconstructed, while for the t-channel only 1, of each, should
+ * exist"), semileptonic final state, same neutrino p_z and same record as hepf_chi2_semilep:
+ *   mode 1, t-channel: chi^2 = ((m_blnu - m_t)/sigma_t)^2 + ((m_lnu - m_W)/sigma_W)^2 over (b, p_z solution); needs one
+ *           lepton and one b-tagged jet; the hadronic fields of the record stay NaN / -1.
+ *   mode 2, Wt: chi^2 = ((m_top - m_t)/sigma_t)^2 + ((m_lnu - m_W)/sigma_W)^2 + ((m_jj - m_W)/sigma_W)^2, the one top being
+ *           the leptonic (b l nu) or the hadronic (b j j) one; over (hypothesis, b, (q1, q2), p_z solution); needs one lepton,
+ *           one b-tagged and two untagged jets; jet_b_lep / m_top_lep are set for a leptonic top, jet_b_had / m_top_had for a
+ *           hadronic one, the other pair stays -1 / NaN.
+ * The dileptonic chi^2 of eq. (1) is not built: the paper's description of it breaks off mid-sentence.
+ */
+int hepf_chi2_single_top(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int mode,
+                         const hepf_chi2_params_t* host_params, hepf_chi2_t* out, void* stream);
 
 /*
  * hepf_histogram — fixed-width histogram of one quantity of the reconstructed events, filled on the device

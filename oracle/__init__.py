@@ -85,6 +85,7 @@ def lib():
         L.orc_quartic.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]
         L.orc_nu_pz.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_void_p]
         L.orc_chi2_semilep.argtypes = [C.POINTER(Events), C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_chi2_single_top.argtypes = [C.POINTER(Events), C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_histogram.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int32, C.c_void_p]
         _lib = L
     return _lib
@@ -286,4 +287,17 @@ def chi2_semilep(store, idx, params=None):
                                 out.ctypes.data, second.ctypes.data)
     if rc != 0:
         raise RuntimeError(f"orc_chi2_semilep: {rc}")
+    return out, second
+
+
+def chi2_single_top(store, idx, mode: int, params=None):
+    """Single-top chi^2 of eq. (1): mode 1 = t-channel, mode 2 = Wt.  (records CHI2_DTYPE[n], second-best chi2 per event)."""
+    ev = events_view(store)
+    idx = np.ascontiguousarray(idx, dtype=np.uint32)
+    out = np.zeros(len(idx), dtype=CHI2_DTYPE); second = np.zeros(len(idx))
+    par = np.asarray(params, dtype=np.float64) if params is not None else None
+    rc = lib().orc_chi2_single_top(C.byref(ev), idx.ctypes.data, len(idx), mode, par.ctypes.data if par is not None else None,
+                                   out.ctypes.data, second.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_chi2_single_top: {rc}")
     return out, second

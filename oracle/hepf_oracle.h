@@ -123,6 +123,9 @@ void orc_default_chi2_params(orc_chi2_params_t* p);
 int orc_nu_pz(const double lep[4], double nux, double nuy, double m_w, double pz[2]);
 int orc_chi2_semilep(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx, const orc_chi2_params_t* params,
                      orc_chi2_t* out, double* out_second);
+/* single-top variants of eq. (1): mode 1 = t-channel (1 top, 1 W), mode 2 = Wt (1 top, 2 W), semileptonic final state */
+int orc_chi2_single_top(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx, int mode, const orc_chi2_params_t* params,
+                        orc_chi2_t* out, double* out_second);
 
 /* histogram of a field of the records (oracle_hist.cpp; pin: numpy restatement + hand-built edge cases) */
 int orc_histogram(const orc_best_t* best, int64_t n, int field, double lo, double hi, int32_t nbins, uint64_t* out);

@@ -79,6 +79,7 @@ def load():
                                     C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_size_t, C.c_void_p]
         L.hepf_chi2_semilep.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.hepf_chi2_single_top.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.hepf_histogram.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
         L.hepf_select_record.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                          C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -415,4 +416,16 @@ def chi2_semilep(events: DeviceEvents, idx, n_idx: int, params=None, *, out=None
     par = (C.c_double * 4)(*params) if params is not None else None
     rc = load().hepf_chi2_semilep(C.byref(ev), idx.data_ptr(), n_idx, par, out.data_ptr(), _stream_ptr(stream))
     _check(rc, "hepf_chi2_semilep")
+    return out[:n_idx]
+
+
+def chi2_single_top(events: DeviceEvents, idx, n_idx: int, mode: int, params=None, *, out=None, stream=None):
+    """hepf_chi2_single_top: mode 1 = t-channel, mode 2 = Wt; uint8 tensor [n_idx, 80] of hepf_chi2_t records."""
+    import torch
+    if out is None:
+        out = torch.empty((max(n_idx, 1), 80), dtype=torch.uint8, device=events.cols.device)
+    ev = events.view()
+    par = (C.c_double * 4)(*params) if params is not None else None
+    rc = load().hepf_chi2_single_top(C.byref(ev), idx.data_ptr(), n_idx, mode, par, out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "hepf_chi2_single_top")
     return out[:n_idx]

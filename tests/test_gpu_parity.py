@@ -662,3 +662,40 @@ def test_cut_stats_and_planned_two_phase_select(hepf):
         hepf.select_planned(dev, cfg.cuts, [0, 1, 2, 3, 4, 5, 6, 6], 4)
     with pytest.raises(hepf.HepfError):
         hepf.plan_chain([(10, 0, 30.0, 1.05)], [0.5])
+
+
+def test_chi2_single_top_parity(hepf):
+    """hepf_chi2_single_top (t-channel = 1 top + 1 W, Wt = 1 top + 2 W) against the oracle: chi^2, p_z and masses to
+    1e-9, indices exact outside near-ties (the oracle's best two within 1e-9), NaN / -1 pattern of the absent top identical."""
+    import torch
+    from paper_2211_14346_b200.binding import CHI2_DTYPE
+    st = hs.generate(30_001, 51, semilep=True, with_truth=False)
+    st.flags[:5000] &= ~np.uint32(0x00020000)            # fewer b-tags in part of the sample
+    mix = hs.generate(30_001, 52, with_truth=False)       # dileptonic events: not applicable
+    st.cols[:, 1::5] = mix.cols[:, 1::5]; st.flags[1::5] = mix.flags[1::5]
+    dev = hepf.DeviceEvents.from_host(st)
+    idx = np.arange(st.n_events, dtype=np.uint32)
+    idx_t = torch.from_numpy(idx.view(np.int32)).cuda()
+    for mode in (1, 2):
+        for par in (None, (170.0, 81.0, 9.0, 6.0)):
+            got = hepf.chi2_single_top(dev, idx_t, len(idx), mode, par).cpu().numpy().reshape(-1).view(CHI2_DTYPE)
+            want, second = oracle.chi2_single_top(st, idx, mode, par)
+            assert np.array_equal(got["event"], want["event"]) and np.array_equal(got["status"], want["status"])
+            assert np.array_equal(got["n_comb"], want["n_comb"])
+            ok = want["status"] == 1
+            assert 0.5 < ok.mean() < 0.9 and np.isnan(got["chi2"][~ok]).all()
+            rel = np.abs(got["chi2"][ok] - want["chi2"][ok]) / np.maximum(1.0, np.abs(want["chi2"][ok]))
+            assert rel.max() <= 1e-9
+            keys = ("jet_b_lep", "jet_b_had", "jet_q1", "jet_q2", "solution")
+            same = np.all([got[k][ok] == want[k][ok] for k in keys], axis=0)
+            tie = (second[ok] - want["chi2"][ok]) <= 1e-9 * np.maximum(1.0, np.abs(want["chi2"][ok]))
+            # Wt with a hadronic top: both p_z solutions satisfy m(l nu) = m_W, the leptonic W term is 0 for both and the chi^2 an
+            # exact tie between them (north_star's near-tie rule): the solution index is then arbitrary, everything else is not
+            assert (same | tie).all() and same.mean() > (0.999 if mode == 1 else 0.8)
+            for f in ("nu_pz", "m_top_lep", "m_top_had", "m_w_lep", "m_w_had"):
+                g, w = got[f][ok][same], want[f][ok][same]
+                assert np.array_equal(np.isnan(g), np.isnan(w)), f
+                fin = ~np.isnan(w)
+                assert (np.abs(g[fin] - w[fin]) <= 1e-9 * np.maximum(1.0, np.abs(w[fin]))).all(), f
+    with pytest.raises(hepf.HepfError):
+        hepf.chi2_single_top(dev, idx_t, 5, 0)
