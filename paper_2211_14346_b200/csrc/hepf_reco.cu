@@ -37,6 +37,8 @@ namespace hepf {
 constexpr int NBM = HEPF_MAX_B;   // candidate slots in the tables
 constexpr int QCAP = 160;          // root stack: <= 31 left over + 4 new roots per lane of a C2 pass (the pass is cut short if it would not fit)
 constexpr int SCAP = 64;          // solve queue: <= 31 left over + 32 new quartics
+constexpr uint32_t TAG_MASK = (1u << 20) - 1u;   // root-stack tag: vv 5 | i 3 | j 3 | h 3 | pair 4 | slot 2
+constexpr uint32_t STAG_MASK = (1u << 11) - 1u;  // solve-queue tag: vv 5 | i 3 | j 3
 
 struct RecoCols {
   const double *lep_px, *lep_py, *lep_pz, *lep_e, *jet_px, *jet_py, *jet_pz, *jet_e, *met_x, *met_y;
@@ -551,7 +553,7 @@ template <int VC, int NBT>
 struct __align__(16) WarpMem {
   static constexpr int NP = NBT * (NBT - 1) / 2;
   double def[3][2 * NBT * VC];   // (d, e, f) of the conic of (leg, candidate, variation); lanes of a pass differ in the variation
-  double fr[FRN - 2][2 * NBT];   // per event: frame of (leg, candidate) without (a, b): c, c1, c2, d1, d2, g1, g2, h1, ile, hml2, hmb2, bln
+  double cc[2 * NBT];            // per event: c of the frame of (leg, candidate)
   double2 pcv[NBT * (NBT - 1)][2];  // per event: pair constants (p2, q1), (r3, 1/h4) of every ordered pairing (128-bit loads)
   double2 ab[2 * NBT];              // per event: (a, b) of the frame of (leg, candidate), read with one 128-bit load
   double ht[VC * NP];            // Higgs term of candidate pair (k, l), k < l
@@ -559,20 +561,31 @@ struct __align__(16) WarpMem {
   double obj[10 * 4];            // nominal (px, py, pz, E)
   double ks[10];                 // kappa * sigma
   double met[2];
-  // solve queue (stage C1 -> C2): depressed quartics that may have real roots, (p, q), (r, aq) and the (variation, i, j) tag
-  double2 s_pq[SCAP], s_ra[SCAP];
-  uint32_t s_tag[SCAP];
-  // root stack (stage C2 -> D): (bits of x, tag) in one 16-byte entry, one STS.128 / LDS.128 per root.
-  // The scales of the ten objects (stages A, M, B, H) live in the same bytes: both queues are empty while a chunk's
-  // tables are built, and the scales are dead once they are.
-  union { ulonglong2 q[QCAP]; double sc_[VC * 10]; };
-  static_assert(sizeof(ulonglong2) * QCAP >= sizeof(double) * VC * 10, "the scales must fit in the root stack's bytes");
+  // Both queues are empty while a chunk's tables are built, and what only the table-building stages (A, M, B, H) read is
+  // dead once they are: the scales of the ten objects and the part of the frames that only stage B uses (c1, c2, d1, d2,
+  // g1, g2, h1, ile, hml2, hmb2, bln; rebuilt at the top of every chunk from the nominal objects — 8 or 12 lanes' work)
+  // live in the queues' bytes.  This is what lets a chunk of 32 variations fit 18 warps on an SM.
+  union {
+    struct {
+      // solve queue (stage C1 -> C2): depressed quartics that may have real roots, (p, q), (r, aq).  The (variation, i, j)
+      // tag of the entry rides in the low 11 bits of aq: aq only shifts the roots (x = t - aq), so this moves the Ferrari
+      // roots by |aq| 2^-41 before they are refined on the conics (the finalize kernel solves the winner's quartic from
+      // unpacked values).  It saves a third array and a load/store per solve.
+      double2 s_pq[SCAP], s_ra[SCAP];
+      // root stack (stage C2 -> D): the Ferrari root x with the 20-bit tag of its cell in the low mantissa bits, one 8-byte
+      // entry per root (x is a starting point: 32 mantissa bits, 2e-10 relative, is finer than the closed form's own
+      // error, and stage D refines it by Newton on the conics).
+      unsigned long long q[QCAP];
+    };
+    struct { double sc_[VC * 10]; double frb[FRN - 3][2 * NBT]; };
+  };
   __device__ __forceinline__ double* sc() { return sc_; }
   __device__ __forceinline__ void push(int at, double x, uint32_t tag) {
-    q[at] = make_ulonglong2((unsigned long long)__double_as_longlong(x), tag);
+    q[at] = ((unsigned long long)__double_as_longlong(x) & ~(unsigned long long)TAG_MASK) | tag;
   }
   __device__ __forceinline__ void pop(int at, double& x, uint32_t& tag) const {
-    const ulonglong2 en = q[at]; x = __longlong_as_double((long long)en.x); tag = (uint32_t)en.y;
+    const unsigned long long en = q[at];
+    x = __longlong_as_double((long long)(en & ~(unsigned long long)TAG_MASK)); tag = (uint32_t)en & TAG_MASK;   // tag bits cleared: x does not depend on its cell
   }
 };
 
@@ -582,8 +595,8 @@ __device__ __forceinline__ void score_entry(const WarpMem<VC, NBT>& W, double x,
   const int vv = tag & 31, i = (tag >> 5) & 7, j = (tag >> 8) & 7, h = (tag >> 11) & 7, t = (tag >> 14) & 15, k = (tag >> 18) & 3;
   const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
   const double2 abA = W.ab[i], abB = W.ab[NBT + j];
-  const Conic A{abA.x, abA.y, W.fr[0][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
-  const Conic B{abB.x, abB.y, W.fr[0][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
+  const Conic A{abA.x, abA.y, W.cc[i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
+  const Conic B{abB.x, abB.y, W.cc[NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
   double y;
   refine_xy(A, B, x, y);
   const double ll = loglik_of(x, y, W.M[vv], W.M[VC + vv], W.ht[t * VC + vv], inv_lambda);
@@ -609,26 +622,9 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   __syncwarp();
   // the n_b = 4 instantiation only ever sees events with four candidates: a compile-time constant there
   const int nb = (NBT == 4) ? 4 : h.n_b, n_pair = nb * (nb - 1) / 2, n_ord = nb * (nb - 1);
-  if (lane < 2 * nb) {               // frames of (leg, candidate): once per event
-    const int leg = lane >= nb, c = lane - leg * nb;
-    const int ls = leg ? 1 - h.lp_slot : h.lp_slot, js = 2 + ((h.cand >> (4 * c)) & 15);
-    const Frame F = make_frame(&W.obj[ls * 4], &W.obj[js * 4]);
-    const int fi = leg * NBT + c;
-    W.ab[fi] = make_double2(F.a, F.b);
-    W.fr[0][fi] = F.c; W.fr[1][fi] = F.c1; W.fr[2][fi] = F.c2;
-    W.fr[3][fi] = F.d1; W.fr[4][fi] = F.d2; W.fr[5][fi] = F.g1; W.fr[6][fi] = F.g2; W.fr[7][fi] = F.h1;
-    W.fr[8][fi] = F.ile; W.fr[9][fi] = F.hml2; W.fr[10][fi] = F.hmb2; W.fr[11][fi] = F.bln;
-  }
-  __syncwarp();
   const uint64_t PK = pair_k_list(nb), PL = pair_l_list(nb);
   // ap / (nb - 1) for ap < nb (nb - 1) as a multiply-shift: /3 -> *11 >> 5 (ap < 12), /4 -> >> 2, /5 -> *13 >> 6 (ap < 30)
   const int dmul = nb == 4 ? 11 : (nb == 5 ? 1 : 13), dsh = nb == 4 ? 5 : (nb == 5 ? 2 : 6);
-  if (lane < n_ord) {                // pair constants of every ordered pairing: once per event
-    const int i = (lane * dmul) >> dsh; int j = lane - i * (nb - 1); j += (j >= i);
-    const PairConst K = pair_consts(W.ab[i].x, W.ab[i].y, W.fr[0][i], W.ab[NBT + j].x, W.ab[NBT + j].y, W.fr[0][NBT + j]);
-    W.pcv[lane][0] = make_double2(K.p2, K.q1); W.pcv[lane][1] = make_double2(K.r3, K.ih4);
-  }
-  __syncwarp();
   const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2), inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
   const unsigned lt = (1u << lane) - 1u;
   const int seedE = seed_scale(P);
@@ -642,6 +638,16 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   for (int v0 = 0; v0 < V; v0 += VC) {
     const int nv = min(VC, V - v0);
     const bool vok = vv < nv;
+    // ---- F: frames of (leg, candidate).  (a, b, c) are kept for the whole event, the rest only until stage B has run.
+    if (lane < 2 * nb) {
+      const int leg = lane >= nb, c = lane - leg * nb;
+      const int ls = leg ? 1 - h.lp_slot : h.lp_slot, js = 2 + ((h.cand >> (4 * c)) & 15);
+      const Frame F = make_frame(&W.obj[ls * 4], &W.obj[js * 4]);
+      const int fi = leg * NBT + c;
+      W.ab[fi] = make_double2(F.a, F.b); W.cc[fi] = F.c;
+      W.frb[0][fi] = F.c1; W.frb[1][fi] = F.c2; W.frb[2][fi] = F.d1; W.frb[3][fi] = F.d2; W.frb[4][fi] = F.g1; W.frb[5][fi] = F.g2;
+      W.frb[6][fi] = F.h1; W.frb[7][fi] = F.ile; W.frb[8][fi] = F.hml2; W.frb[9][fi] = F.hmb2; W.frb[10][fi] = F.bln;
+    }
     // ---- A: normals -> scales ---------------------------------------------------------------------------------------
     for (int b0 = 0; b0 < h.nblk; b0 += LPB) {
       const int blk = b0 + sub;
@@ -654,6 +660,11 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       }
     }
     __syncwarp();
+    if (v0 == 0 && lane < n_ord) {     // pair constants of every ordered pairing: once per event
+      const int i = (lane * dmul) >> dsh; int j = lane - i * (nb - 1); j += (j >= i);
+      const PairConst K = pair_consts(W.ab[i].x, W.ab[i].y, W.cc[i], W.ab[NBT + j].x, W.ab[NBT + j].y, W.cc[NBT + j]);
+      W.pcv[lane][0] = make_double2(K.p2, K.q1); W.pcv[lane][1] = make_double2(K.r3, K.ih4);
+    }
     // ---- M: MET' = MET - sum_t (s_t - 1) pT_t, summed in slot order ----------------------------------------------------
 #pragma unroll 1
     for (int c0 = 0; c0 < 2; c0 += LPB) {
@@ -675,9 +686,9 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         const int ls = leg ? 1 - h.lp_slot : h.lp_slot, js = 2 + ((h.cand >> (4 * c)) & 15);
         const int fi = leg * NBT + c;
         Frame F;
-        F.a = W.ab[fi].x; F.b = W.ab[fi].y; F.c = W.fr[0][fi]; F.c1 = W.fr[1][fi]; F.c2 = W.fr[2][fi];
-        F.d1 = W.fr[3][fi]; F.d2 = W.fr[4][fi]; F.g1 = W.fr[5][fi]; F.g2 = W.fr[6][fi]; F.h1 = W.fr[7][fi];
-        F.ile = W.fr[8][fi]; F.hml2 = W.fr[9][fi]; F.hmb2 = W.fr[10][fi]; F.bln = W.fr[11][fi];
+        F.a = W.ab[fi].x; F.b = W.ab[fi].y; F.c = W.cc[fi]; F.c1 = W.frb[0][fi]; F.c2 = W.frb[1][fi];
+        F.d1 = W.frb[2][fi]; F.d2 = W.frb[3][fi]; F.g1 = W.frb[4][fi]; F.g2 = W.frb[5][fi]; F.h1 = W.frb[6][fi];
+        F.ile = W.frb[7][fi]; F.hml2 = W.frb[8][fi]; F.hmb2 = W.frb[9][fi]; F.bln = W.frb[10][fi];
         Conic q; double c0_;
         q.a = F.a; q.b = F.b; q.c = F.c;
         const double sl = W.sc()[ls * VC + vv], sb = W.sc()[js * VC + vv];
@@ -716,8 +727,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
           const int i = (ap * dmul) >> dsh; int j = ap - i * (nb - 1); j += (j >= i);   // i = ap / (nb - 1)
           const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
           const double2 abA = W.ab[i], abB = W.ab[NBT + j], k01 = W.pcv[ap][0], k23 = W.pcv[ap][1];
-          const Conic A{abA.x, abA.y, W.fr[0][i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
-          const Conic B{abB.x, abB.y, W.fr[0][NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
+          const Conic A{abA.x, abA.y, W.cc[i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
+          const Conic B{abB.x, abB.y, W.cc[NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
           const PairConst K{k01.x, k01.y, k23.x, k23.y};
           double g3, g2, g1, g0;
           resultant(A, B, K, g3, g2, g1, g0);
@@ -728,7 +739,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         const unsigned bk = __ballot_sync(0xffffffffu, keep);
         if (keep) {
           const int at = sn + __popc(bk & lt);
-          W.s_pq[at] = make_double2(qp, qq); W.s_ra[at] = make_double2(qr, qaq); W.s_tag[at] = stag;
+          const double aqt = __hiloint2double(__double2hiint(qaq), (int)(((uint32_t)__double2loint(qaq) & ~STAG_MASK) | stag));
+          W.s_pq[at] = make_double2(qp, qq); W.s_ra[at] = make_double2(qr, aqt);
         }
         sn += __popc(bk);
         __syncwarp();
@@ -741,8 +753,9 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
           double xa[2], xb[2];
           if (lane < take) {
             const double2 pq = W.s_pq[sn + lane], ra = W.s_ra[sn + lane];
-            const uint32_t st = W.s_tag[sn + lane];
-            mask = ferrari(pq.x, pq.y, ra.x, ra.y, seedE, xa, xb);
+            const uint32_t st = (uint32_t)__double2loint(ra.y) & STAG_MASK;
+            const double aq = __hiloint2double(__double2hiint(ra.y), (int)((uint32_t)__double2loint(ra.y) & ~STAG_MASK));   // tag bits cleared
+            mask = ferrari(pq.x, pq.y, ra.x, aq, seedE, xa, xb);
             if (mask) {
               double ht; int hh, kk, ll;
               best_higgs<NBT, VC>(&W.ht[st & 31], nb, (st >> 5) & 7, (st >> 8) & 7, ht, hh, kk, ll);
@@ -1007,16 +1020,16 @@ static int launch_search(const RecoCols& cols, const uint32_t* idx, const int64_
 }
 
 // both candidate-count classes: n_b = 4 (tables for 4 candidates, more warps per SM) and n_b = 5, 6
-template <int VC4, int VC6, int RW, int MINB4, int MINB6>
+template <int VC4, int VC6, int RW4, int RW6, int MINB4, int MINB6>
 static int launch_search_both(const RecoCols& cols, const uint32_t* idx, const int64_t* n_dev, int64_t n_idx, int V, uint64_t seed,
                               const hepf_tth_params_t& P, uint2* winners, cudaStream_t stream) {
   unsigned long long* counters = reinterpret_cast<unsigned long long*>(winners + n_idx);   // two group counters
   HEPF_CUDA_TRY(cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), stream));
   timing_mark(T_RECO0, stream);
-  int rc = launch_search<VC4, 4, RW, MINB4>(cols, idx, n_dev, n_idx, V, seed, P, winners, counters, stream);
+  int rc = launch_search<VC4, 4, RW4, MINB4>(cols, idx, n_dev, n_idx, V, seed, P, winners, counters, stream);
   timing_mark(T_RECO1, stream);
   if (rc != HEPF_OK) return rc;
-  rc = launch_search<VC6, 6, RW, MINB6>(cols, idx, n_dev, n_idx, V, seed, P, winners, counters + 1, stream);
+  rc = launch_search<VC6, 6, RW6, MINB6>(cols, idx, n_dev, n_idx, V, seed, P, winners, counters + 1, stream);
   timing_mark(T_RECO2, stream);
   return rc;
 }
@@ -1069,8 +1082,12 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, con
                       events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags,
                       events->n_events, events->stride, events->event_base, event_out_offset};
   uint2* winners = reinterpret_cast<uint2*>(ws);
-  if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 12, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
-  else rc = launch_search_both<16, 8, 2, 10, 9>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
+  // chunk of variations per pass of the pipeline: 32 when that wastes at most an eighth of the lanes of the last chunk,
+  // else 16 or 8.  32 (16 for n_b = 6) needs so much shared memory per warp that one block of 18 (19) warps fills an SM.
+  const int waste32 = ((n_variations + 31) & ~31) - n_variations;
+  if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 2, 12, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
+  else if (8 * waste32 > n_variations) rc = launch_search_both<16, 8, 2, 2, 10, 9>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
+  else rc = launch_search_both<32, 16, 18, 19, 1, 1>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
   if (rc != HEPF_OK) return rc;
   int dev = 0, sms = 148;
   HEPF_CUDA_TRY(cudaGetDevice(&dev));
