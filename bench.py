@@ -59,6 +59,19 @@ def load_profiled_ops() -> dict:
     return d
 
 
+def search_kernel_name(V: int, nb6: bool) -> str:
+    """The instantiation hepf_reconstruct_tth launches for V variations (hepf_reco.cu, reconstruct_impl): chunks of 32 variations
+    (16 for n_b = 5, 6) unless that wastes more than an eighth of the last chunk's lanes, then 16 (8), and 8 for V <= 8."""
+    waste32 = ((V + 31) & ~31) - V
+    if V <= 8:
+        vc4, vc6 = 8, 8
+    elif 8 * waste32 > V:
+        vc4, vc6 = 16, 8
+    else:
+        vc4, vc6 = 32, 16
+    return f"reco_search_kernel<{vc6},6>" if nb6 else f"reco_search_kernel<{vc4},4>"
+
+
 def chain_bytes_per_event(chain) -> int:
     """Algorithmic bytes hepf_select must read per event: flags + the columns the chain names."""
     need = set()
@@ -316,7 +329,7 @@ class TthRun:
         """FP64 lane-op roofline of the dominant search kernel + HBM roofline of select_eval."""
         km = self.kernel_ms
         nb6 = km["search6"] > km["search4"]
-        name = "reco_search_kernel<16,6>" if nb6 else ("reco_search_kernel<16,4>" if self.V > 8 else "reco_search_kernel<8,4>")
+        name = search_kernel_name(self.V, nb6)
         ms_search = km["search6"] if nb6 else km["search4"]
         lane_peak = sms * FP64_LANES_PER_SM * sm_max_mhz * 1e6
         entry = prof["kernels"].get(name) if prof.get("current") else None

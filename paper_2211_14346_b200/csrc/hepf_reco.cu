@@ -557,6 +557,8 @@ struct __align__(16) WarpMem {
   double2 pcv[NBT * (NBT - 1)][2];  // per event: pair constants (p2, q1), (r3, 1/h4) of every ordered pairing (128-bit loads)
   double2 ab[2 * NBT];              // per event: (a, b) of the frame of (leg, candidate), read with one 128-bit load
   double ht[VC * NP];            // Higgs term of candidate pair (k, l), k < l
+  double hm2[NBT];               // per event: nominal m^2 of candidate c
+  double hdot[NP];               // per event: 2 (b_k . b_l) of the nominal candidates k < l (Minkowski product)
   double M[VC * 2];              // MET'
   double obj[10 * 4];            // nominal (px, py, pz, E)
   double ks[10];                 // kappa * sigma
@@ -611,6 +613,7 @@ template <int VC, int NBT>
 __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const RecoCols& ev, const EventHead& h, int V, uint32_t k0,
                                                  uint32_t k1, const hepf_tth_params_t& P, int lane) {
   constexpr int LPB = 32 / VC;     // item sub-groups per warp pass
+  constexpr bool FUSE_M = (LPB == 1);   // a lane owns a variation: MET' is accumulated in stage A
   const int vv = lane & (VC - 1), sub = lane / VC;
   // ---- prologue: nominal objects, kappa*sigma, MET ------------------------------------------------------------------
   if (lane < 10) {
@@ -625,6 +628,17 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
   const uint64_t PK = pair_k_list(nb), PL = pair_l_list(nb);
   // ap / (nb - 1) for ap < nb (nb - 1) as a multiply-shift: /3 -> *11 >> 5 (ap < 12), /4 -> >> 2, /5 -> *13 >> 6 (ap < 30)
   const int dmul = nb == 4 ? 11 : (nb == 5 ? 1 : 13), dsh = nb == 4 ? 5 : (nb == 5 ? 2 : 6);
+  // Higgs-pair constants: (s_k b_k + s_l b_l)^2 = s_k^2 m_k^2 + s_l^2 m_l^2 + s_k s_l 2 (b_k . b_l), so a variation costs
+  // three products and three fused operations per pair instead of two scaled four-vectors, their sum and its square
+  if (lane < n_pair) {
+    const int kk = (int)(PK >> (4 * lane)) & 15, ll = (int)(PL >> (4 * lane)) & 15;
+    const double* bk = &W.obj[(2 + ((h.cand >> (4 * kk)) & 15)) * 4];
+    const double* bl = &W.obj[(2 + ((h.cand >> (4 * ll)) & 15)) * 4];
+    W.hdot[pair_index<NBT>(kk, ll)] = 2.0 * fma(bk[3], bl[3], -fma(bk[0], bl[0], fma(bk[1], bl[1], bk[2] * bl[2])));
+  } else if (lane >= 16 && lane < 16 + nb) {
+    const double* b = &W.obj[(2 + ((h.cand >> (4 * (lane - 16))) & 15)) * 4];
+    W.hm2[lane - 16] = fma(b[3], b[3], -fma(b[0], b[0], fma(b[1], b[1], b[2] * b[2])));
+  }
   const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2), inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
   const unsigned lt = (1u << lane) - 1u;
   const int seedE = seed_scale(P);
@@ -648,7 +662,10 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       W.frb[0][fi] = F.c1; W.frb[1][fi] = F.c2; W.frb[2][fi] = F.d1; W.frb[3][fi] = F.d2; W.frb[4][fi] = F.g1; W.frb[5][fi] = F.g2;
       W.frb[6][fi] = F.h1; W.frb[7][fi] = F.ile; W.frb[8][fi] = F.hml2; W.frb[9][fi] = F.hmb2; W.frb[10][fi] = F.bln;
     }
-    // ---- A: normals -> scales ---------------------------------------------------------------------------------------
+    // ---- A: normals -> scales.  With 32 variations per chunk a lane owns a variation and walks its blocks, i.e. its objects,
+    //      in slot order: MET' = MET - sum_t (s_t - 1) pT_t is then accumulated on the way (the objects past 2 + n_jet have a
+    //      zero four-vector and s = 1: they add +0, which leaves the sum's bits alone) and stage M is not needed.
+    double ax = 0.0, ay = 0.0;
     for (int b0 = 0; b0 < h.nblk; b0 += LPB) {
       const int blk = b0 + sub;
       if (vok && blk < h.nblk) {
@@ -657,8 +674,14 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         double ze, zo; block_normals(x, ze, zo);
         const double s0 = scale_of(W.ks[2 * blk], ze, P.s_min), s1 = scale_of(W.ks[2 * blk + 1], zo, P.s_min);
         W.sc()[(2 * blk) * VC + vv] = s0; W.sc()[(2 * blk + 1) * VC + vv] = s1;
+        if (FUSE_M) {
+          const double d0 = __dadd_rn(s0, -1.0), d1 = __dadd_rn(s1, -1.0);
+          ax = __dadd_rn(ax, __dmul_rn(d0, W.obj[8 * blk])); ay = __dadd_rn(ay, __dmul_rn(d0, W.obj[8 * blk + 1]));
+          ax = __dadd_rn(ax, __dmul_rn(d1, W.obj[8 * blk + 4])); ay = __dadd_rn(ay, __dmul_rn(d1, W.obj[8 * blk + 5]));
+        }
       }
     }
+    if (FUSE_M && vok) { W.M[vv] = __dadd_rn(W.met[0], -ax); W.M[VC + vv] = __dadd_rn(W.met[1], -ay); }
     __syncwarp();
     if (v0 == 0 && lane < n_ord) {     // pair constants of every ordered pairing: once per event
       const int i = (lane * dmul) >> dsh; int j = lane - i * (nb - 1); j += (j >= i);
@@ -667,7 +690,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
     }
     // ---- M: MET' = MET - sum_t (s_t - 1) pT_t, summed in slot order ----------------------------------------------------
 #pragma unroll 1
-    for (int c0 = 0; c0 < 2; c0 += LPB) {
+    for (int c0 = 0; c0 < (FUSE_M ? 0 : 2); c0 += LPB) {
       const int comp = c0 + sub;
       if (vok && comp < 2) {
         double acc = 0.0;
@@ -676,7 +699,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         W.M[comp * VC + vv] = __dadd_rn(W.met[comp], -acc);
       }
     }
-    __syncwarp();
+    if (!FUSE_M) __syncwarp();
     // ---- B: leg conics (leg 0: l+ with candidate c; leg 1: l- with candidate c, shifted by MET') -------------------------
 #pragma unroll 1
     for (int c0 = 0; c0 < 2 * nb; c0 += LPB) {
@@ -705,9 +728,13 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       if (vok && p < n_pair) {
         const int kk = (int)(PK >> (4 * p)) & 15, ll = (int)(PL >> (4 * p)) & 15;
         const int j1 = 2 + ((h.cand >> (4 * kk)) & 15), j2 = 2 + ((h.cand >> (4 * ll)) & 15);
-        const V4 b1 = scale_v4(&W.obj[j1 * 4], W.sc()[j1 * VC + vv]), b2 = scale_v4(&W.obj[j2 * 4], W.sc()[j2 * VC + vv]);
-        const double t = (mass_of(b1.e + b2.e, b1.x + b2.x, b1.y + b2.y, b1.z + b2.z) - P.m_higgs) * inv_sh;
-        W.ht[pair_index<NBT>(kk, ll) * VC + vv] = -0.5 * (t * t);
+        const int pi = pair_index<NBT>(kk, ll);
+        const double sk = W.sc()[j1 * VC + vv], sl = W.sc()[j2 * VC + vv];
+        const double m2 = fma(sk * sk, W.hm2[kk], fma(sl * sl, W.hm2[ll], (sk * sl) * W.hdot[pi]));
+        // a NaN (garbage inputs: inf - inf) stays a NaN, so that such a pair never wins here while the finalize kernel, which
+        // adds the four-vectors, finds no finite mass for it
+        const double t = (sqrt_fast(m2 < 0.0 ? 0.0 : m2) - P.m_higgs) * inv_sh;
+        W.ht[pi * VC + vv] = -0.5 * (t * t);
       }
     }
     __syncwarp();
@@ -721,21 +748,20 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       const bool last = a0 >= n_ord;
       if (!last) {
         const int ap = a0 + sub;
-        bool keep = false;
-        double qp = 0.0, qq = 0.0, qr = 0.0, qaq = 0.0; uint32_t stag = 0;
-        if (vok && ap < n_ord) {
-          const int i = (ap * dmul) >> dsh; int j = ap - i * (nb - 1); j += (j >= i);   // i = ap / (nb - 1)
-          const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
-          const double2 abA = W.ab[i], abB = W.ab[NBT + j], k01 = W.pcv[ap][0], k23 = W.pcv[ap][1];
-          const Conic A{abA.x, abA.y, W.cc[i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
-          const Conic B{abB.x, abB.y, W.cc[NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
-          const PairConst K{k01.x, k01.y, k23.x, k23.y};
-          double g3, g2, g1, g0;
-          resultant(A, B, K, g3, g2, g1, g0);
-          depress(g3, g2, g1, g0, qaq, qp, qq, qr);
-          keep = !certainly_no_real_root(qp, qq, qr);
-          stag = (uint32_t)vv | (i << 5) | (j << 8);
-        }
+        // Every lane computes (no branch, no default values): a lane without an item (variation past V, or pairing past the last
+        // one when the sub-groups do not divide their number) works on whatever its table slot holds — the indices stay inside
+        // the warp's tables — and is not kept.
+        const int i = (ap * dmul) >> dsh; int j = ap - i * (nb - 1); j += (j >= i);   // i = ap / (nb - 1)
+        const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
+        const double2 abA = W.ab[i], abB = W.ab[NBT + j], k01 = W.pcv[ap][0], k23 = W.pcv[ap][1];
+        const Conic A{abA.x, abA.y, W.cc[i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
+        const Conic B{abB.x, abB.y, W.cc[NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
+        const PairConst K{k01.x, k01.y, k23.x, k23.y};
+        double g3, g2, g1, g0, qp, qq, qr, qaq;
+        resultant(A, B, K, g3, g2, g1, g0);
+        depress(g3, g2, g1, g0, qaq, qp, qq, qr);
+        const bool keep = !certainly_no_real_root(qp, qq, qr) && vok && ap < n_ord;
+        const uint32_t stag = (uint32_t)vv | (i << 5) | (j << 8);
         const unsigned bk = __ballot_sync(0xffffffffu, keep);
         if (keep) {
           const int at = sn + __popc(bk & lt);
