@@ -13,7 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libhepf_oracle.so")
-_SRCS = ["oracle_philox.cpp", "oracle_select.cpp", "oracle_reco.cpp", "oracle_hist.cpp", "oracle_chi2.cpp"]
+_SRCS = ["oracle_philox.cpp", "oracle_select.cpp", "oracle_reco.cpp", "oracle_hist.cpp", "oracle_chi2.cpp", "oracle_chi2_dilep.cpp"]
 
 
 def build(force: bool = False) -> str:
@@ -301,3 +301,44 @@ def chi2_single_top(store, idx, mode: int, params=None):
     if rc != 0:
         raise RuntimeError(f"orc_chi2_single_top: {rc}")
     return out, second
+
+
+CHI2_DILEP_DTYPE = np.dtype([("chi2", "f8"), ("nu", "f8", 3), ("nubar", "f8", 3), ("m_top", "f8"), ("m_antitop", "f8"),
+                             ("m_wplus", "f8"), ("m_wminus", "f8"), ("jet_b", "i4"), ("jet_bbar", "i4"), ("grid_x", "i4"),
+                             ("grid_y", "i4"), ("sol_nu", "i4"), ("sol_nubar", "i4"), ("n_comb", "i4"), ("status", "u4"),
+                             ("event", "u4"), ("pad_", "i4")])
+assert CHI2_DILEP_DTYPE.itemsize == 128
+
+
+class Split(C.Structure):
+    _fields_ = [("split_range", C.c_double), ("split_n", C.c_int32), ("pad_", C.c_int32)]
+
+
+def chi2_dilep(store, idx, params=None, split=None, n_threads: int = 1):
+    """Dileptonic chi^2 of eq. (1) (oracle_chi2_dilep.cpp).  split = (split_range, split_n) or None (160 GeV, 32).
+    Returns (records CHI2_DILEP_DTYPE[n], second-best chi2 per event)."""
+    ev = events_view(store)
+    idx = np.ascontiguousarray(idx, dtype=np.uint32)
+    out = np.zeros(len(idx), dtype=CHI2_DILEP_DTYPE); second = np.zeros(len(idx))
+    par = np.asarray(params, dtype=np.float64) if params is not None else None
+    sp = Split(float(split[0]), int(split[1]), 0) if split is not None else None
+    L = lib()
+    L.orc_chi2_dilep.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+    rc = L.orc_chi2_dilep(C.byref(ev), idx.ctypes.data, len(idx), par.ctypes.data if par is not None else None,
+                          C.byref(sp) if sp is not None else None, out.ctypes.data, second.ctypes.data, int(n_threads))
+    if rc != 0:
+        raise RuntimeError(f"orc_chi2_dilep failed: {rc}")
+    return out, second
+
+
+def chi2_dilep_point(store, e: int, slot_b: int, slot_bbar: int, nux: float, nuy: float, params=None):
+    """chi^2 of one hypothesis at one split of the MET: (chi2[2][2] over the p_z solutions, pz_nu[2], pz_nubar[2])."""
+    ev = events_view(store)
+    par = np.asarray(params, dtype=np.float64) if params is not None else None
+    out = np.zeros(4); p1 = np.zeros(2); p2 = np.zeros(2)
+    L = lib()
+    L.orc_chi2_dilep_point.argtypes = [C.c_void_p, C.c_uint32, C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p,
+                                       C.c_void_p, C.c_void_p, C.c_void_p]
+    L.orc_chi2_dilep_point(C.byref(ev), int(e), int(slot_b), int(slot_bbar), float(nux), float(nuy),
+                           par.ctypes.data if par is not None else None, out.ctypes.data, p1.ctypes.data, p2.ctypes.data)
+    return out.reshape(2, 2), p1, p2

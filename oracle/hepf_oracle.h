@@ -23,6 +23,9 @@
  *   O4 score / argmax ........ prefix property in V, sigma_scale = 0, z-rotation invariance, slot permutation
  *   chi2 (semileptonic) ...... p_z against a dense scan of m(l nu), truth recovery in closure mode (chi2 = 0 at the true
  *                              combination), brute-force enumeration in numpy, permutation invariance
+ *   chi2 (dileptonic) ........ chi2 = 0 at the generator's true neutrinos and pairing (closure mode) and at the roots of the
+ *                              pinned dilepton solve (orc_solve_pairing); the grid argmin against a Python loop over
+ *                              orc_chi2_dilep_point; 90-degree rotation about z maps the grid onto itself
  *   histogram ................ hand-built edge cases (lower edge in, upper edge overflow, NaN, unsolved), numpy restatement
  *   PARITY UNPINNED against the paper: the likelihood formula, sigma_H, lambda_nu, the resolution model
  *   and the 8-cut thresholds are definitions of this build (R3, R7, R10), not paper values.
@@ -126,6 +129,21 @@ int orc_chi2_semilep(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx,
 /* single-top variants of eq. (1): mode 1 = t-channel (1 top, 1 W), mode 2 = Wt (1 top, 2 W), semileptonic final state */
 int orc_chi2_single_top(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx, int mode, const orc_chi2_params_t* params,
                         orc_chi2_t* out, double* out_second);
+
+/* chi^2 reconstruction of DILEPTONIC ttbar (oracle_chi2_dilep.cpp, reading R15 of DESIGN.md): the neutrino's
+ * transverse momentum is scanned over a split_n x split_n grid of half-width split_range around MET/2, the antineutrino
+ * takes the rest of the MET, each p_z follows from its W as in the semileptonic case */
+typedef struct { double split_range; int32_t split_n, pad_; } orc_split_t;
+typedef struct {
+  double chi2, nu[3], nubar[3], m_top, m_antitop, m_wplus, m_wminus;
+  int32_t jet_b, jet_bbar, grid_x, grid_y, sol_nu, sol_nubar, n_comb;
+  uint32_t status, event; int32_t pad_;
+} orc_chi2_dilep_t;   /* 128 bytes */
+void orc_default_split(orc_split_t* s);
+int orc_chi2_dilep_point(const orc_events_t* ev, uint32_t e, int sb, int sbbar, double nux, double nuy,
+                         const orc_chi2_params_t* params, double out[4], double pz_nu[2], double pz_nubar[2]);
+int orc_chi2_dilep(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx, const orc_chi2_params_t* params,
+                   const orc_split_t* split, orc_chi2_dilep_t* out, double* out_second, int n_threads);
 
 /* histogram of a field of the records (oracle_hist.cpp; pin: numpy restatement + hand-built edge cases) */
 int orc_histogram(const orc_best_t* best, int64_t n, int field, double lo, double hi, int32_t nbins, uint64_t* out);

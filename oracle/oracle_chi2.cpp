@@ -114,7 +114,7 @@ extern "C" int orc_chi2_semilep(const orc_events_t* ev, const uint32_t* idx, int
 //           solution; needs one lepton, one b-tag and two untagged jets.
 // Enumeration order (hypothesis, b, (q1, q2), solution), strict <.  Record: jet_b_lep = the b-jet if the top is leptonic else
 // -1, jet_b_had likewise; m_top_lep / m_top_had NaN for the top that is not there; t-channel: no hadronic entries at all.
-// The dileptonic chi^2 of eq. (1) is not built: PAPER.md:329 breaks off in the middle of its description (R14).
+// The dileptonic chi^2 of eq. (1) is in oracle_chi2_dilep.cpp (PAPER.md:329 breaks off in the middle of its description: reading R15).
 extern "C" int orc_chi2_single_top(const orc_events_t* ev, const uint32_t* idx, int64_t n_idx, int mode,
                                    const orc_chi2_params_t* params, orc_chi2_t* out, double* out_second) {
   if (!ev || (n_idx > 0 && !idx) || n_idx < 0 || !out || (mode != 1 && mode != 2)) return -1;
