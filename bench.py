@@ -7,7 +7,7 @@ for every surviving event.  `value` counts event x variation x pairing solves pe
 HBM; `e2e` is the same metric through hepf_tth_host (host buffers in, results out, copies inside the timed region).
 The default run also times the other configs of BASELINE.json (cfg3, cfg4, cfg5) and reports them under `configs`.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg1|cfg2|cfg3|cfg4|cfg5|chi2]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg1|cfg2|cfg3|cfg4|cfg5|chi2|chi2_dilep]
 Under torchrun every rank runs its own shard (events keyed by global index, no data-path collective): weak scaling.
 Everything printed is measured in this run, except the per-solve FP64 instruction counts and the DRAM traffic of the
 search kernels, which only ncu can count: they are read from profiles/r02_fp64_ops.json and used only if that file's hash
@@ -166,6 +166,42 @@ def run_chi2(args):
                       "gpu_launches": args.steps,
                       "roofline": {"bound": "hbm", "kernel": "chi2_semilep_kernel", "achieved": gbs, "peak": hbm, "unit": "GB/s",
                                    "frac": gbs / hbm, "traffic": None, "algorithmic_bytes": by, "peak_source": src}}))
+
+
+def run_chi2_dilep(args):
+    """--workload chi2_dilep: hepf_chi2_dilep (eq. 1, dileptonic final state; R15) on the cfg2 generator's
+    events: a 32 x 32 scan of the MET split per event, 12 ordered b pairs, up to 4 p_z combinations per point."""
+    import torch
+    import paper_2211_14346_b200 as hepf
+    from paper_2211_14346_b200.binding import CHI2_DILEP_DTYPE
+    hepf.load()
+    torch.cuda.set_device(0)
+    n = args.events or 200_000
+    st = hs.generate(n, 12, with_truth=False)
+    dev = hepf.DeviceEvents.from_host(st)
+    idx_t = torch.arange(n, dtype=torch.int32, device="cuda")
+    out = torch.empty((n, 128), dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+    W = max(3, args.warmup)
+    for _ in range(W):
+        hepf.chi2_dilep(dev, idx_t, n, out=out, stream=stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        hepf.chi2_dilep(dev, idx_t, n, out=out, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    rec = out.cpu().numpy().reshape(-1).view(CHI2_DILEP_DTYPE)
+    combos = float(rec["n_comb"].astype(np.int64).sum())
+    print(json.dumps({"metric": "chi2-reconstructed dileptonic ttbar events/sec (32 x 32 MET-split scan)", "value": n / (ms * 1e-3),
+                      "unit": "events/s", "n_gpus": 1, "steps": args.steps, "warmup": W, "ms_per_step": ms, "higher_is_better": True,
+                      "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": f"chi2_dilep: {n} dileptonic events, 4 b-tags, split grid 32 x 32 over +-160 GeV",
+                                 "l2": "FP64-bound: one event (about 350 B) per warp and 1024 grid points of arithmetic; nothing to flush"},
+                      "gpu_launches": args.steps, "chi2_evaluations_per_s": combos / (ms * 1e-3),
+                      "grid_points_per_s": 1024.0 * float((rec["status"] == 1).sum()) / (ms * 1e-3)}))
 
 
 def solves_of(store, idx, n_variations: int) -> int:
@@ -421,7 +457,7 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="hepf", choices=["hepf", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "chi2"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "chi2", "chi2_dilep"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra-configs", action="store_true", help="skip the cfg3 / cfg4 / cfg5 lines of the default run")
@@ -432,6 +468,8 @@ def main():
         return run_philox(args)
     if args.workload == "chi2":
         return run_chi2(args)
+    if args.workload == "chi2_dilep":
+        return run_chi2_dilep(args)
     cfg = hs.CONFIGS[int(args.workload[3])]
     if args.impl == "reference":
         return run_reference(args, cfg, args.workload)

@@ -242,6 +242,30 @@ int hepf_chi2_single_top(const hepf_events_t* events, const uint32_t* idx, int64
                          const hepf_chi2_params_t* host_params, hepf_chi2_t* out, void* stream);
 
 /*
+ * hepf_chi2_dilep — the dileptonic ttbar case of eq. (1) ("for the dileptonic final states, two neutrinos
+ * must be fully reconstructed.  This implies, splitting the E_T^miss between the two neutrinos and determine, using the mass
+ * constraints from the chi^2" — the sentence breaks off there; R15 is the reading).  The neutrino's transverse
+ * momentum is scanned over a split_n x split_n grid, nu_T = MET/2 + split_range (u_gx, u_gy) with u_g = (2 g + 1)/split_n - 1,
+ * the antineutrino takes nubar_T = MET - nu_T; each p_z follows from its W as in hepf_chi2_semilep (two roots of m(l nu) = m_W,
+ * else the p_z of closest approach); chi^2 = [t_top^2 + t_W^2](l+, nu, b) + [t_top^2 + t_W^2](l-, nubar, bbar) over ordered
+ * pairs (b, bbar) of the first 4 b-tagged jet slots; first minimum in the order (b, bbar, gx, gy, solution of nu, of nubar).
+ *   idx          device uint32[n_idx] event indices of the view (an index >= n_events gives status 2 | 8).
+ *   host_params  HOST pointer or NULL (172.5, 80.4, 11.5, 7.5);  host_split  HOST pointer or NULL (160 GeV, 32).
+ *   out          device hepf_chi2_dilep_t[n_idx], 16-byte aligned.  status 1 = reconstructed, 2 = not applicable (n_lep != 2,
+ *                same-sign leptons or fewer than two b-tags), 0 = no finite chi^2 anywhere; NaN / -1 payload unless status 1.
+ *                n_comb = number of (b, bbar, grid point, solutions) combinations evaluated.
+ * Errors: HEPF_ERR_ARG for NULL / misaligned pointers, non-positive widths, split_n outside 1..64, split_range < 0.
+ */
+typedef struct { double split_range; int32_t split_n, pad_; } hepf_split_t;
+typedef struct {
+  double chi2, nu[3], nubar[3], m_top, m_antitop, m_wplus, m_wminus;
+  int32_t jet_b, jet_bbar, grid_x, grid_y, sol_nu, sol_nubar, n_comb;
+  uint32_t status, event; int32_t pad_;
+} hepf_chi2_dilep_t;   /* 128 bytes */
+int hepf_chi2_dilep(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, const hepf_chi2_params_t* host_params,
+                    const hepf_split_t* host_split, hepf_chi2_dilep_t* out, void* stream);
+
+/*
  * hepf_histogram — fixed-width histogram of one quantity of the reconstructed events, filled on the device
  * (App. 8.2: the user's finalize() writes histograms of reconstructed quantities; PAPER.md:278:
  * per-cut variable recording).  Only records with status bit 0 (has a solution) are filled.

@@ -80,6 +80,7 @@ def load():
                                     C.c_size_t, C.c_void_p]
         L.hepf_chi2_semilep.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.hepf_chi2_single_top.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.hepf_chi2_dilep.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.hepf_histogram.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
         L.hepf_select_record.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                          C.c_void_p, C.c_double, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -428,4 +429,30 @@ def chi2_single_top(events: DeviceEvents, idx, n_idx: int, mode: int, params=Non
     par = (C.c_double * 4)(*params) if params is not None else None
     rc = load().hepf_chi2_single_top(C.byref(ev), idx.data_ptr(), n_idx, mode, par, out.data_ptr(), _stream_ptr(stream))
     _check(rc, "hepf_chi2_single_top")
+    return out[:n_idx]
+
+
+CHI2_DILEP_DTYPE = np.dtype([("chi2", "f8"), ("nu", "f8", 3), ("nubar", "f8", 3), ("m_top", "f8"), ("m_antitop", "f8"),
+                             ("m_wplus", "f8"), ("m_wminus", "f8"), ("jet_b", "i4"), ("jet_bbar", "i4"), ("grid_x", "i4"),
+                             ("grid_y", "i4"), ("sol_nu", "i4"), ("sol_nubar", "i4"), ("n_comb", "i4"), ("status", "u4"),
+                             ("event", "u4"), ("pad_", "i4")])
+assert CHI2_DILEP_DTYPE.itemsize == 128
+
+
+class _Split(C.Structure):
+    _fields_ = [("split_range", C.c_double), ("split_n", C.c_int32), ("pad_", C.c_int32)]
+
+
+def chi2_dilep(events: DeviceEvents, idx, n_idx: int, params=None, split=None, *, out=None, stream=None):
+    """hepf_chi2_dilep: uint8 tensor [n_idx, 128] of hepf_chi2_dilep_t records (see CHI2_DILEP_DTYPE); params = (m_top, m_w,
+    sigma_top, sigma_w) or None; split = (split_range, split_n) or None (160 GeV, 32)."""
+    import torch
+    ev = events.view()
+    if out is None:
+        out = torch.empty((max(n_idx, 1), 128), dtype=torch.uint8, device=events.cols.device)
+    par = (C.c_double * 4)(*params) if params is not None else None
+    sp = _Split(float(split[0]), int(split[1]), 0) if split is not None else None
+    rc = load().hepf_chi2_dilep(C.byref(ev), idx.data_ptr(), n_idx, par, C.byref(sp) if sp is not None else None,
+                                out.data_ptr(), _stream_ptr(stream))
+    _check(rc, "hepf_chi2_dilep")
     return out[:n_idx]

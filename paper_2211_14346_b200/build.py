@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhepf.so")
-SOURCES = ["hepf_api.cu", "hepf_philox.cu", "hepf_select.cu", "hepf_reco.cu", "hepf_host.cu", "hepf_hist.cu", "hepf_chi2.cu"]
+SOURCES = ["hepf_api.cu", "hepf_philox.cu", "hepf_select.cu", "hepf_reco.cu", "hepf_host.cu", "hepf_hist.cu", "hepf_chi2.cu", "hepf_chi2_dilep.cu"]
 # hepf_reco.cu spells every fused multiply-add itself: no contraction, so that the search and the finalize kernel
 # (and any two builds) evaluate the shared device functions to the same bits
 EXTRA_FLAGS = {"hepf_reco.cu": ["-fmad=false"]}

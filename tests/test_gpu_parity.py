@@ -699,3 +699,54 @@ def test_chi2_single_top_parity(hepf):
                 assert (np.abs(g[fin] - w[fin]) <= 1e-9 * np.maximum(1.0, np.abs(w[fin]))).all(), f
     with pytest.raises(hepf.HepfError):
         hepf.chi2_single_top(dev, idx_t, 5, 0)
+
+
+def test_chi2_dilep_parity(hepf):
+    """hepf_chi2_dilep (eq. 1, dileptonic; R15) against oracle/oracle_chi2_dilep.cpp: status,
+    n_comb and (outside near-ties of the oracle's two best values) every index exactly, chi^2 / momenta / masses to 1e-9."""
+    import torch
+    from paper_2211_14346_b200.binding import CHI2_DILEP_DTYPE
+
+    def run(st, idx, par=None, split=None):
+        dev = hepf.DeviceEvents.from_host(st)
+        idx_t = torch.from_numpy(np.ascontiguousarray(idx, dtype=np.uint32).view(np.int32)).cuda()
+        got = hepf.chi2_dilep(dev, idx_t, len(idx), par, split).cpu().numpy().reshape(-1).view(CHI2_DILEP_DTYPE)
+        want, second = oracle.chi2_dilep(st, idx, par, split, n_threads=16)
+        assert np.array_equal(got["status"], want["status"]) and np.array_equal(got["event"], want["event"])
+        assert np.array_equal(got["n_comb"], want["n_comb"])
+        ok = want["status"] == 1
+        dead = ~ok
+        assert np.isnan(got["chi2"][dead]).all() and (got["jet_b"][dead] == -1).all() and (got["grid_x"][dead] == -1).all()
+        g, w = got[ok], want[ok]
+        assert np.all(np.abs(g["chi2"] - w["chi2"]) <= 1e-9 * np.maximum(1.0, w["chi2"]))
+        tie = second[ok] <= w["chi2"] * (1 + 1e-9) + 1e-12
+        keys = ("jet_b", "jet_bbar", "grid_x", "grid_y", "sol_nu", "sol_nubar")
+        same = np.all([g[f] == w[f] for f in keys], axis=0)
+        assert (same | tie).all(), np.flatnonzero(~(same | tie))[:5]
+        for f in ("nu", "nubar"):
+            sc = np.maximum(1.0, np.abs(w[f]).max(axis=1))
+            assert np.all(np.abs(g[f][same] - w[f][same]).max(axis=1) <= 1e-9 * sc[same])
+        for f in ("m_top", "m_antitop", "m_wplus", "m_wminus"):
+            assert np.all(np.abs(g[f][same] - w[f][same]) <= 1e-9 * np.maximum(1.0, w[f][same]))
+        return int(ok.sum()), int(same.sum())
+
+    st = hs.generate(1500, 51, with_truth=False)
+    n_ok, n_same = run(st, np.arange(1500))
+    assert n_ok == 1500 and n_same >= n_ok - 2
+    # closure mode on an odd grid (the centre cell is MET/2), a ragged index list, other parameters
+    cl = hs.generate(601, 52, closure=True, with_truth=False)
+    n_ok, _ = run(cl, np.arange(1, 601, 2), (170.0, 81.0, 9.0, 6.0), (120.0, 7))
+    assert n_ok == 300
+    # mixed sample: semileptonic events, same-sign pairs and single-tag events are "not applicable"
+    mix = hs.generate(800, 53, with_truth=False)
+    sl = hs.generate(800, 54, semilep=True, with_truth=False)
+    mix.cols[:, 1::2] = sl.cols[:, 1::2]; mix.flags[1::2] = sl.flags[1::2]
+    mix.flags[0:100:4] |= np.uint32((1 << 4) | (1 << 5))
+    n_ok, _ = run(mix, np.arange(800), None, (160.0, 16))
+    assert 0 < n_ok < 400
+    dev = hepf.DeviceEvents.from_host(mix)
+    idx_t = torch.arange(8, dtype=torch.int32, device="cuda")
+    assert hepf.chi2_dilep(dev, idx_t, 0).shape[0] == 0
+    for bad in ((160.0, 0), (160.0, 65), (-1.0, 8)):
+        with pytest.raises(hepf.HepfError):
+            hepf.chi2_dilep(dev, idx_t, 8, None, bad)
