@@ -161,9 +161,11 @@ size_t hepf_select_planned_workspace_bytes(int64_t n_events);
  *   n_idx        host value.
  *   host_params  host pointer or NULL.
  *   out_best     device hepf_best_t[n_idx], 16-byte aligned; out_best[k] belongs to idx[k].
- *   ws           device workspace >= hepf_reconstruct_workspace_bytes(n_idx, n_variations), 8-byte aligned (one
- *                8-byte winner key per listed event, written by the search kernels and read by the finalize kernel,
- *                plus two 8-byte work counters).
+ *   ws           device workspace >= hepf_reconstruct_workspace_bytes(n_idx, n_variations), 8-byte aligned: one
+ *                8-byte winner key per listed event, written by the search kernels and read by the finalize kernel, two
+ *                8-byte work counters, and 42 columns of n_idx doubles in which the search kernels leave the nominal
+ *                objects of the events they reconstructed (344 bytes per listed event in all), so that the finalize
+ *                kernel reads them coalesced instead of gathering them from the store again.
  */
 int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
                          uint64_t seed, const hepf_tth_params_t* host_params, hepf_best_t* out_best, void* ws,

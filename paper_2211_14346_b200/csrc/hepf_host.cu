@@ -21,6 +21,34 @@ constexpr int64_t MIN_CHUNK = 32768;      // events; smaller samples are not wor
 
 size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 
+// Chunks of consecutive events; boundaries are multiples of 4 so that every chunk view keeps the 16-byte alignment.  Chunk
+// c covers events [start[c], start[c + 1]).  The first and the last chunks are smaller (weights 1 2 4 5 ... 5 4 2 1): the
+// kernels cannot start before the first chunk has arrived, and what remains to be done after the last byte has arrived —
+// the last chunk's kernels and its copy back — is what the pipeline cannot hide.  Returns the number of chunks.
+int chunk_plan(int64_t n, int64_t* start) {
+  int nc = (int)(n / MIN_CHUNK); if (nc < 1) nc = 1; if (nc > MAX_CHUNKS) nc = MAX_CHUNKS;
+  int wsum = 0, w[MAX_CHUNKS];
+  for (int c = 0; c < nc; c++) {
+    const int edge = c < nc - 1 - c ? c : nc - 1 - c;
+    w[c] = (nc >= 6 && edge < 3) ? (1 << edge) : 5;
+    wsum += w[c];
+  }
+  int64_t acc = 0; start[0] = 0;
+  for (int c = 0; c < nc; c++) {
+    acc += w[c];
+    int64_t e = (n * acc / wsum + 3) / 4 * 4;
+    start[c + 1] = (c + 1 == nc || e > n) ? n : e;
+  }
+  return nc;
+}
+int64_t longest_chunk(int64_t n) {
+  int64_t start[MAX_CHUNKS + 1];
+  const int nc = chunk_plan(n, start);
+  int64_t m = 1;
+  for (int c = 0; c < nc; c++) if (start[c + 1] - start[c] > m) m = start[c + 1] - start[c];
+  return m;
+}
+
 struct ArenaLayout { size_t cols, flags, idx, count, cutflow, sel_ws[2], reco_ws[2], best, total; };
 
 ArenaLayout layout(int64_t n, int64_t stride) {
@@ -33,7 +61,7 @@ ArenaLayout layout(int64_t n, int64_t stride) {
   L.cutflow = off; off += up256((size_t)MAX_CHUNKS * HEPF_MAX_CUTS * sizeof(int64_t));
   for (int k = 0; k < 2; k++) {      // one set per compute stream (chunks alternate between two streams)
     L.sel_ws[k] = off; off += up256(hepf_select_workspace_bytes(n));
-    L.reco_ws[k] = off; off += up256(hepf_reconstruct_workspace_bytes(n, 1));
+    L.reco_ws[k] = off; off += up256(hepf_reconstruct_workspace_bytes(longest_chunk(n), 1));   // per chunk: winner keys + nominal objects
   }
   L.best = off; off += up256((size_t)(n > 0 ? n : 1) * sizeof(hepf_best_t));
   L.total = off;
@@ -120,26 +148,8 @@ extern "C" int hepf_tth_host(const hepf_events_t* hev, const hepf_cut_t* host_cu
   const int rows[16] = {2, 2, 2, 2, 2, 2, 8, 8, 8, 8, 8, 8, 1, 1, 1, 1};
   const double* dptr[16];
   { int64_t row = 0; for (int b = 0; b < 16; b++) { dptr[b] = dcols + row * dstride; row += rows[b]; } }
-  // chunks of consecutive events; boundaries are multiples of 4 so that every chunk view keeps the 16-byte alignment
-  int nc = (int)(n / MIN_CHUNK); if (nc < 1) nc = 1; if (nc > MAX_CHUNKS) nc = MAX_CHUNKS;
-  // chunk c covers events [start[c], start[c + 1]).  The first and the last chunks are smaller (weights 1 2 4 5 ... 5 4 2 1):
-  // the kernels cannot start before the first chunk has arrived, and what remains to be done after the last byte has
-  // arrived — the last chunk's kernels and its copy back — is what the pipeline cannot hide.
   int64_t start[MAX_CHUNKS + 1];
-  {
-    int wsum = 0, w[MAX_CHUNKS];
-    for (int c = 0; c < nc; c++) {
-      const int edge = c < nc - 1 - c ? c : nc - 1 - c;
-      w[c] = (nc >= 6 && edge < 3) ? (1 << edge) : 5;
-      wsum += w[c];
-    }
-    int64_t acc = 0; start[0] = 0;
-    for (int c = 0; c < nc; c++) {
-      acc += w[c];
-      int64_t e = (n * acc / wsum + 3) / 4 * 4;
-      start[c + 1] = (c + 1 == nc || e > n) ? n : e;
-    }
-  }
+  const int nc = chunk_plan(n, start);
   // one 64-row copy per chunk when the host columns are the rows of one [64][stride] block in the device block's row order
   // (the layout hepf_synth and DeviceEvents use); otherwise one copy per column group
   bool one_block = true;
@@ -182,7 +192,7 @@ extern "C" int hepf_tth_host(const hepf_events_t* hev, const hepf_cut_t* host_cu
     HEPF_PIPE_TRY(cudaMemcpyAsync(g_pipe.counts + c, dcount + c, sizeof(int64_t), cudaMemcpyDeviceToHost, cs_));
     HEPF_PIPE_TRY(cudaEventRecord(g_pipe.counted[c], cs_));
     rc = reconstruct_impl(&view, didx + lo, dcount + c, len, n_variations, seed, host_params, dbest + lo, base + L.reco_ws[w],
-                          up256(hepf_reconstruct_workspace_bytes(n, 1)), cs_, lo);
+                          up256(hepf_reconstruct_workspace_bytes(longest_chunk(n), 1)), cs_, lo);
     if (rc != HEPF_OK) return drain(rc, stream);
     if (lo > 0) {
       add_offset_kernel<<<256, 256, 0, cs_>>>(didx + lo, dcount + c, (uint32_t)lo);

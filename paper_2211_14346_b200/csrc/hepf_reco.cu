@@ -36,6 +36,7 @@ namespace hepf {
 
 constexpr int NBM = HEPF_MAX_B;   // candidate slots in the tables
 constexpr int QCAP = 160;          // root stack: <= 31 left over + 4 new roots per lane of a C2 pass (the pass is cut short if it would not fit)
+constexpr int NOMINAL_ROWS = 42;   // workspace copy of an event's nominal objects: 10 x (px, py, pz, E) + MET x, y
 constexpr int SCAP = 64;          // solve queue: <= 31 left over + 32 new quartics
 constexpr uint32_t TAG_MASK = (1u << 20) - 1u;   // root-stack tag: vv 5 | i 3 | j 3 | h 3 | pair 4 | slot 2
 constexpr uint32_t STAG_MASK = (1u << 11) - 1u;  // solve-queue tag: vv 5 | i 3 | j 3
@@ -391,10 +392,11 @@ struct DD { double hi, lo; };
 __device__ __forceinline__ DD dd_fast2sum(double a, double b) { const double s = a + b; return DD{s, b - (s - a)}; }
 __device__ __forceinline__ DD dd_2sum(double a, double b) { const double s = a + b, v = s - a; return DD{s, (a - (s - v)) + (b - v)}; }
 __device__ __forceinline__ DD dd_2prod(double a, double b) { const double p = a * b; return DD{p, fma(a, b, -p)}; }
+// double-double sum: the high parts exactly, the low parts in plain FP64 (error <= 2^-105 (|a| + |b|): the residuals below
+// are needed to about 2^-80 of their largest term)
 __device__ __forceinline__ DD dd_add(DD a, DD b) {
-  DD s = dd_2sum(a.hi, b.hi); const DD t = dd_2sum(a.lo, b.lo);
-  s = dd_fast2sum(s.hi, s.lo + t.hi);
-  return dd_fast2sum(s.hi, s.lo + t.lo);
+  const DD s = dd_2sum(a.hi, b.hi);
+  return dd_fast2sum(s.hi, s.lo + (a.lo + b.lo));
 }
 __device__ __forceinline__ DD dd_neg(DD a) { return DD{-a.hi, -a.lo}; }
 __device__ __forceinline__ DD dd_sub(DD a, DD b) { return dd_add(a, dd_neg(b)); }
@@ -409,47 +411,57 @@ __device__ __forceinline__ DD dd_sqrt(DD a) {
 __device__ __forceinline__ DD dd_dot4(const V4& u, const V4& v) {
   return dd_sub(dd_2prod(u.e, v.e), dd_add(dd_add(dd_2prod(u.x, v.x), dd_2prod(u.y, v.y)), dd_2prod(u.z, v.z)));
 }
-// residuals of one leg: (l + n)^2 - m_W^2 and (l + n + b)^2 - m_t^2 for the massless n = (p, |p|)
-__device__ __forceinline__ void dd_leg_residuals(const V4& l, const V4& b, const DD p[3], DD E, DD mw2, DD mt2, double& fw, double& ft) {
+// residuals of one leg: (l + n)^2 - m_W^2 and (l + n + b)^2 - m_t^2 for the massless n = (p, |p|).  w0 = m_l^2 - m_W^2 and
+// t0 = (l + b)^2 - m_t^2 do not depend on n: they are formed once per polish.
+__device__ __forceinline__ void dd_leg_consts(const V4& l, const V4& b, DD mw2, DD mt2, DD& w0, DD& t0) {
   const DD ml2 = dd_dot4(l, l), mb2 = dd_dot4(b, b), lb = dd_dot4(l, b);
+  w0 = dd_sub(ml2, mw2);
+  t0 = dd_sub(dd_add(dd_add(ml2, mb2), dd_add(lb, lb)), mt2);
+}
+__device__ __forceinline__ void dd_leg_residuals(const V4& l, const V4& b, const DD p[3], DD E, DD w0, DD t0, double& fw, double& ft) {
   const DD lp = dd_sub(dd_muld(E, l.e), dd_add(dd_add(dd_muld(p[0], l.x), dd_muld(p[1], l.y)), dd_muld(p[2], l.z)));
   const DD bp = dd_sub(dd_muld(E, b.e), dd_add(dd_add(dd_muld(p[0], b.x), dd_muld(p[1], b.y)), dd_muld(p[2], b.z)));
-  const DD w = dd_sub(dd_add(ml2, dd_add(lp, lp)), mw2);                       // m_l^2 + 2 l.n - m_W^2
-  DD t = dd_add(dd_add(ml2, mb2), dd_add(lb, lb));                            // (l + b)^2
-  t = dd_sub(dd_add(t, dd_add(dd_add(lp, lp), dd_add(bp, bp))), mt2);         // + 2 (l + b).n - m_t^2
+  const DD w = dd_add(w0, dd_add(lp, lp));                                    // m_l^2 + 2 l.n - m_W^2
+  const DD t = dd_add(t0, dd_add(dd_add(lp, lp), dd_add(bp, bp)));            // (l + b)^2 + 2 (l + b).n - m_t^2
   fw = w.hi + w.lo; ft = t.hi + t.lo;
 }
 // Returns false (and leaves the point alone) if the iteration does not settle next to where it started.
 __device__ __noinline__ bool polish_raw(const V4 lp, const V4 bi, const V4 lm, const V4 bj, double Mx, double My, double m_top,
                                         double m_w, double& x, double& y, double& pz, double& qx, double& qy, double& qz) {
   const DD mw2 = dd_2prod(m_w, m_w), mt2 = dd_2prod(m_top, m_top);
+  DD w01, t01, w02, t02;
+  dd_leg_consts(lp, bi, mw2, mt2, w01, t01); dd_leg_consts(lm, bj, mw2, mt2, w02, t02);
   DD u[4] = {DD{x, 0.0}, DD{y, 0.0}, DD{pz, 0.0}, DD{qz, 0.0}};
   const double scale = fabs(x) + fabs(y) + fabs(pz) + fabs(qz);
   double mv = CUDART_INF, total = 0.0;
+  // A step of size mv leaves an error of about C mv^2 + (rounding of the FP64 Jacobian, 1e-15) mv: once a step is below
+  // 1e-10 of the scale the point is converged far beyond the 1e-9 the record is compared at, and no further residual
+  // evaluation is spent on confirming it.  The usual case is ONE step (the search's FP64 point is 1e-12 .. 1e-15 away).
 #pragma unroll 1
-  for (int it = 0; it < 6 && mv > 1e-24 * scale; it++) {
+  for (int it = 0; it < 6 && mv > 1e-10 * scale; it++) {
     const DD q[3] = {dd_sub(DD{Mx, 0.0}, u[0]), dd_sub(DD{My, 0.0}, u[1]), u[3]};
     const DD p[3] = {u[0], u[1], u[2]};
     const DD E = dd_sqrt(dd_add(dd_add(dd_mul(p[0], p[0]), dd_mul(p[1], p[1])), dd_mul(p[2], p[2])));
     const DD Eq = dd_sqrt(dd_add(dd_add(dd_mul(q[0], q[0]), dd_mul(q[1], q[1])), dd_mul(q[2], q[2])));
     double A[4][5];
-    dd_leg_residuals(lp, bi, p, E, mw2, mt2, A[0][4], A[1][4]);
-    dd_leg_residuals(lm, bj, q, Eq, mw2, mt2, A[2][4], A[3][4]);
-    const double ie = 1.0 / E.hi, iq = 1.0 / Eq.hi;
+    dd_leg_residuals(lp, bi, p, E, w01, t01, A[0][4], A[1][4]);
+    dd_leg_residuals(lm, bj, q, Eq, w02, t02, A[2][4], A[3][4]);
+    const double ie = rcp_fast(E.hi), iq = rcp_fast(Eq.hi);
     const double ux = p[0].hi * ie, uy = p[1].hi * ie, uz = p[2].hi * ie, vx = q[0].hi * iq, vy = q[1].hi * iq, vz = q[2].hi * iq;
     const double s1 = lp.e, s2 = lp.e + bi.e, t1 = lm.e, t2 = lm.e + bj.e;
     A[0][0] = 2.0 * (s1 * ux - lp.x); A[0][1] = 2.0 * (s1 * uy - lp.y); A[0][2] = 2.0 * (s1 * uz - lp.z); A[0][3] = 0.0;
     A[1][0] = 2.0 * (s2 * ux - (lp.x + bi.x)); A[1][1] = 2.0 * (s2 * uy - (lp.y + bi.y)); A[1][2] = 2.0 * (s2 * uz - (lp.z + bi.z)); A[1][3] = 0.0;
     A[2][0] = -2.0 * (t1 * vx - lm.x); A[2][1] = -2.0 * (t1 * vy - lm.y); A[2][2] = 0.0; A[2][3] = 2.0 * (t1 * vz - lm.z);
     A[3][0] = -2.0 * (t2 * vx - (lm.x + bj.x)); A[3][1] = -2.0 * (t2 * vy - (lm.y + bj.y)); A[3][2] = 0.0; A[3][3] = 2.0 * (t2 * vz - (lm.z + bj.z));
-    // Gaussian elimination with partial pivoting (rows swapped in place)
+    // Gaussian elimination with partial pivoting (rows swapped in place); the step only has to be good to a few digits
+    double ipv[4];
     for (int c = 0; c < 4; c++) {
       int pr = c;
       for (int r = c + 1; r < 4; r++) if (fabs(A[r][c]) > fabs(A[pr][c])) pr = r;
       for (int k = 0; k < 5; k++) { const double t = A[c][k]; A[c][k] = A[pr][k]; A[pr][k] = t; }
-      const double ip = 1.0 / A[c][c];
+      ipv[c] = rcp_fast(A[c][c]);
       for (int r = c + 1; r < 4; r++) {
-        const double m = A[r][c] * ip;
+        const double m = A[r][c] * ipv[c];
         for (int k = c; k < 5; k++) A[r][k] -= m * A[c][k];
       }
     }
@@ -457,14 +469,14 @@ __device__ __noinline__ bool polish_raw(const V4 lp, const V4 bi, const V4 lm, c
     for (int c = 3; c >= 0; c--) {
       double sacc = A[c][4];
       for (int k = c + 1; k < 4; k++) sacc -= A[c][k] * d[k];
-      d[c] = sacc / A[c][c];
+      d[c] = sacc * ipv[c];
     }
     mv = fabs(d[0]) + fabs(d[1]) + fabs(d[2]) + fabs(d[3]);
     total += mv;
     if (!(total <= 1e-3 * scale)) return false;     // NaN, or wandering off to another intersection
     for (int c = 0; c < 4; c++) u[c] = dd_sub(u[c], DD{d[c], 0.0});
   }
-  if (!(mv <= 1e-18 * scale)) return false;
+  if (!(mv <= 1e-10 * scale)) return false;
   const DD fqx = dd_sub(DD{Mx, 0.0}, u[0]), fqy = dd_sub(DD{My, 0.0}, u[1]);
   x = u[0].hi; y = u[1].hi; pz = u[2].hi; qz = u[3].hi; qx = fqx.hi; qy = fqy.hi;
   return true;
@@ -840,7 +852,7 @@ __device__ __forceinline__ int64_t list_length(const int64_t* n_dev, int64_t n_c
 template <int VC, int NBT, int RW, int MINB>
 __global__ void __launch_bounds__(32 * RW, MINB)
 reco_search_kernel(RecoCols ev, const uint32_t* __restrict__ idx, const int64_t* __restrict__ n_dev, int64_t n_cap, int epc, int V,
-                   uint32_t k0, uint32_t k1, hepf_tth_params_t P, uint2* __restrict__ winners,
+                   uint32_t k0, uint32_t k1, hepf_tth_params_t P, uint2* __restrict__ winners, double* __restrict__ nominal,
                    unsigned long long* __restrict__ next_group) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   WarpMem<VC, NBT>& W = reinterpret_cast<WarpMem<VC, NBT>*>(smem_raw)[threadIdx.x >> 5];
@@ -866,14 +878,19 @@ reco_search_kernel(RecoCols ev, const uint32_t* __restrict__ idx, const int64_t*
       const EventHead h = load_head(ev, (int64_t)__ldg(idx + k));
       const uint32_t key = search_event<VC, NBT>(W, ev, h, V, k0, k1, P, lane);
       if (lane == 0) winners[k] = make_uint2(key, key != 0xffffffffu ? 1u : 0u);
+      // The nominal objects and the MET of the event, as this warp gathered them, go to the workspace as 42 columns of
+      // n_cap doubles: the finalize kernel then reads them coalesced instead of gathering 40 scattered 64-byte DRAM atoms per
+      // event a second time (the selected events are a few per cent of the store).
+      for (int it = lane; it < NOMINAL_ROWS; it += 32) nominal[(int64_t)it * n_cap + k] = it < 40 ? W.obj[it] : W.met[it - 40];
       __syncwarp();
     }
   }
 }
 
 // One selected event: re-derive the winner in full, polish it and write the record.
-__device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_t* __restrict__ idx, int64_t k, uint32_t k0, uint32_t k1,
-                                               const hepf_tth_params_t& P, const uint2* __restrict__ winners, hepf_best_t* __restrict__ out) {
+__device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_t* __restrict__ idx, int64_t k, int64_t n_cap, uint32_t k0,
+                                               uint32_t k1, const hepf_tth_params_t& P, const uint2* __restrict__ winners,
+                                               const double* __restrict__ nominal, hepf_best_t* __restrict__ out) {
   const EventHead h = load_head(ev, (int64_t)__ldg(idx + k));
   const uint2 w = winners[k];
   hepf_best_t* o = out + k;
@@ -888,8 +905,20 @@ __device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_
   const int v = (int)(w.x >> 11), a6 = (w.x >> 5) & 63, i = a6 / 6, j = a6 - 6 * i, hsel = (w.x >> 2) & 7, ksel = w.x & 3;
   const int nb = h.n_b;
   const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
+  // Nominal objects and MET from the workspace copy the search kernel left (42 columns of n_cap doubles: consecutive
+  // threads read consecutive addresses), not from the store, where every value of a selected event is its own DRAM atom.
+  double obj[10][4], sc[10], ksv[10];
+#pragma unroll
+  for (int t = 0; t < 10; t++)
+#pragma unroll
+    for (int c = 0; c < 4; c++) obj[t][c] = __ldcs(nominal + (int64_t)(4 * t + c) * n_cap + k);
+  const double met_x = __ldcs(nominal + 40 * n_cap + k), met_y = __ldcs(nominal + 41 * n_cap + k);
+#pragma unroll
+  for (int t = 0; t < 10; t++) {       // kappa * sigma as load_object computes it (step 2)
+    const double sigma = t < 2 ? P.lep_sigma : __dadd_rn(__ddiv_rn(P.jet_stoch, __dsqrt_rn(obj[t][3])), P.jet_const);
+    ksv[t] = t < 2 + h.n_jet ? __dmul_rn(P.sigma_scale, sigma) : 0.0;
+  }
   // smear this variation
-  double obj[10][4], sc[10];
   double ax = 0.0, ay = 0.0;
   for (int blk = 0; blk < h.nblk; blk++) {
     uint32_t x[4];
@@ -897,17 +926,14 @@ __device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_
     double z[2]; block_normals(x, z[0], z[1]);
     for (int u = 0; u < 2; u++) {
       const int t = 2 * blk + u;
-      double ks = 0.0;
-      if (t < 2 + h.n_jet) load_object(ev, h.e, t, P, obj[t], ks);
-      else obj[t][0] = obj[t][1] = obj[t][2] = obj[t][3] = 0.0;
-      sc[t] = scale_of(ks, z[u], P.s_min);
+      sc[t] = scale_of(ksv[t], z[u], P.s_min);
       if (t < 2 + h.n_jet) {
         const double d = __dadd_rn(sc[t], -1.0);
         ax = __dadd_rn(ax, __dmul_rn(d, obj[t][0])); ay = __dadd_rn(ay, __dmul_rn(d, obj[t][1]));
       }
     }
   }
-  const double Mx = __dadd_rn(__ldg(ev.met_x + h.e), -ax), My = __dadd_rn(__ldg(ev.met_y + h.e), -ay);
+  const double Mx = __dadd_rn(met_x, -ax), My = __dadd_rn(met_y, -ay);
   const int lps = h.lp_slot, lms = 1 - h.lp_slot;
   const int si = (h.cand >> (4 * i)) & 15, sj = (h.cand >> (4 * j)) & 15;
   const V4 lp = scale_v4(obj[lps], sc[lps]), lm = scale_v4(obj[lms], sc[lms]);
@@ -965,10 +991,11 @@ __device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_
 // One thread per listed event (grid-stride: the grid is sized from the capacity, the length may live on the device).
 __global__ void __launch_bounds__(128, 4)   // 128 registers: the kernel is a chain of dependent FP64 operations, more resident warps hide it
 reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, const int64_t* __restrict__ n_dev, int64_t n_cap, uint32_t k0,
-                     uint32_t k1, hepf_tth_params_t P, const uint2* __restrict__ winners, hepf_best_t* __restrict__ out) {
+                     uint32_t k1, hepf_tth_params_t P, const uint2* __restrict__ winners, const double* __restrict__ nominal,
+                     hepf_best_t* __restrict__ out) {
   const int64_t n_idx = list_length(n_dev, n_cap);
   for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_idx; k += (int64_t)gridDim.x * blockDim.x)
-    finalize_event(ev, idx, k, k0, k1, P, winners, out);
+    finalize_event(ev, idx, k, n_cap, k0, k1, P, winners, nominal, out);
 }
 
 // hepf_tth_system: invariant mass and transverse momentum of the reconstructed ttH system of each record (PAPER.md:410-442,
@@ -1017,7 +1044,7 @@ tth_system_kernel(RecoCols ev, const hepf_best_t* __restrict__ best, int64_t n, 
 
 template <int VC, int NBT, int RW, int MINB>
 static int launch_search(const RecoCols& cols, const uint32_t* idx, const int64_t* n_dev, int64_t n_idx, int V, uint64_t seed,
-                         const hepf_tth_params_t& P, uint2* winners, unsigned long long* counter, cudaStream_t stream) {
+                         const hepf_tth_params_t& P, uint2* winners, double* nominal, unsigned long long* counter, cudaStream_t stream) {
   const size_t smem = sizeof(WarpMem<VC, NBT>) * RW;
   auto kern = reco_search_kernel<VC, NBT, RW, MINB>;
   static thread_local int blocks_per_sm = 0, sms = 0, cached_dev = -1;   // per instantiation (smem is a constant of it) and device
@@ -1039,7 +1066,7 @@ static int launch_search(const RecoCols& cols, const uint32_t* idx, const int64_
   const int64_t n_groups = (n_idx + epc - 1) / epc;
   const int64_t want = (n_groups + RW - 1) / RW, cap = (int64_t)sms * blocks_per_sm;
   const unsigned grid = (unsigned)(want < cap ? want : cap);
-  kern<<<grid, 32 * RW, smem, stream>>>(cols, idx, n_dev, n_idx, epc, V, (uint32_t)seed, (uint32_t)(seed >> 32), P, winners, counter);
+  kern<<<grid, 32 * RW, smem, stream>>>(cols, idx, n_dev, n_idx, epc, V, (uint32_t)seed, (uint32_t)(seed >> 32), P, winners, nominal, counter);
   count_launch();
   HEPF_CUDA_TRY(cudaGetLastError());
   return HEPF_OK;
@@ -1048,14 +1075,14 @@ static int launch_search(const RecoCols& cols, const uint32_t* idx, const int64_
 // both candidate-count classes: n_b = 4 (tables for 4 candidates, more warps per SM) and n_b = 5, 6
 template <int VC4, int VC6, int RW4, int RW6, int MINB4, int MINB6>
 static int launch_search_both(const RecoCols& cols, const uint32_t* idx, const int64_t* n_dev, int64_t n_idx, int V, uint64_t seed,
-                              const hepf_tth_params_t& P, uint2* winners, cudaStream_t stream) {
+                              const hepf_tth_params_t& P, uint2* winners, double* nominal, cudaStream_t stream) {
   unsigned long long* counters = reinterpret_cast<unsigned long long*>(winners + n_idx);   // two group counters
   HEPF_CUDA_TRY(cudaMemsetAsync(counters, 0, 2 * sizeof(unsigned long long), stream));
   timing_mark(T_RECO0, stream);
-  int rc = launch_search<VC4, 4, RW4, MINB4>(cols, idx, n_dev, n_idx, V, seed, P, winners, counters, stream);
+  int rc = launch_search<VC4, 4, RW4, MINB4>(cols, idx, n_dev, n_idx, V, seed, P, winners, nominal, counters, stream);
   timing_mark(T_RECO1, stream);
   if (rc != HEPF_OK) return rc;
-  rc = launch_search<VC6, 6, RW6, MINB6>(cols, idx, n_dev, n_idx, V, seed, P, winners, counters + 1, stream);
+  rc = launch_search<VC6, 6, RW6, MINB6>(cols, idx, n_dev, n_idx, V, seed, P, winners, nominal, counters + 1, stream);
   timing_mark(T_RECO2, stream);
   return rc;
 }
@@ -1064,10 +1091,17 @@ static int launch_search_both(const RecoCols& cols, const uint32_t* idx, const i
 
 using namespace hepf;
 
+static size_t nominal_offset(int64_t n_idx) {
+  const size_t n = (size_t)(n_idx > 0 ? n_idx : 1);
+  return (n * sizeof(uint2) + 16 + 15) / 16 * 16;
+}
+
 extern "C" size_t hepf_reconstruct_workspace_bytes(int64_t n_idx, int32_t n_variations) {
   (void)n_variations;
   if (n_idx < 0) return 0;
-  return (size_t)(n_idx > 0 ? n_idx : 1) * sizeof(uint2) + 16;   // one winner key per listed event + two work counters
+  // one winner key per listed event + two work counters, then the nominal objects of the searched events (42 columns)
+  const size_t n = (size_t)(n_idx > 0 ? n_idx : 1);
+  return nominal_offset(n_idx) + (size_t)NOMINAL_ROWS * n * sizeof(double);
 }
 
 extern "C" int hepf_reconstruct_tth(const hepf_events_t* events, const uint32_t* idx, int64_t n_idx, int32_t n_variations,
@@ -1108,19 +1142,20 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, con
                       events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags,
                       events->n_events, events->stride, events->event_base, event_out_offset};
   uint2* winners = reinterpret_cast<uint2*>(ws);
+  double* nominal = reinterpret_cast<double*>(static_cast<char*>(ws) + nominal_offset(n_idx));
   // chunk of variations per pass of the pipeline: 32 when that wastes at most an eighth of the lanes of the last chunk,
   // else 16 or 8.  32 (16 for n_b = 6) needs so much shared memory per warp that one block of 18 (19) warps fills an SM.
   const int waste32 = ((n_variations + 31) & ~31) - n_variations;
-  if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 2, 12, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
-  else if (8 * waste32 > n_variations) rc = launch_search_both<16, 8, 2, 2, 10, 9>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
-  else rc = launch_search_both<32, 16, 18, 19, 1, 1>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, stream);
+  if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 2, 12, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
+  else if (8 * waste32 > n_variations) rc = launch_search_both<16, 8, 2, 2, 10, 9>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
+  else rc = launch_search_both<32, 16, 18, 19, 1, 1>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
   if (rc != HEPF_OK) return rc;
   int dev = 0, sms = 148;
   HEPF_CUDA_TRY(cudaGetDevice(&dev));
   HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   const int64_t want = (n_idx + 127) / 128, cap = (int64_t)sms * 32;
   reco_finalize_kernel<<<(unsigned)(want < cap ? want : cap), 128, 0, stream>>>(cols, idx, n_dev, n_idx, (uint32_t)seed,
-                                                                             (uint32_t)(seed >> 32), P, winners, out_best);
+                                                                             (uint32_t)(seed >> 32), P, winners, nominal, out_best);
   count_launch();
   timing_mark(T_RECO3, stream);
   HEPF_CUDA_TRY(cudaGetLastError());
