@@ -304,7 +304,7 @@ __device__ __forceinline__ int ferrari(double p, double q, double r, double aq, 
   if (!(fabs(step) <= 1e-8 * m)) m = resolvent_rescue(m, p, tp, c1, c0);
   int mask = 0;
   if (m > 0.0) {
-    const double s = sqrt_fast(2.0 * m), qs = q * rcp_fast(s);          // 2 qs' with qs' = q / (2 s)
+    double is_; const double s = sqrt_rcp_fast(2.0 * m, is_), qs = q * is_;   // 2 qs' with qs' = q / (2 s); 1 / s comes with the root
     const double base = -2.0 * (m + p);
     const double dA = fma(-2.0, qs, base), dB = fma(2.0, qs, base);
     if (dA >= 0.0) { const double sq = sqrt_fast(dA); xa[0] = fma(0.5, s + sq, -aq); xa[1] = fma(0.5, s - sq, -aq); mask |= 1; }

@@ -573,6 +573,14 @@ def test_garbage_inputs_terminate_and_keep_the_status_contract(hepf):
     assert (c["status"] == 2).all()                                      # dileptonic sample: not applicable
     h = hepf.histogram(hepf.reconstruct_tth(dev, idx_t, n, 8, 5), n, "loglik", -50.0, 10.0, 32).cpu().numpy()
     assert 0 < int(h.sum()) <= int(solved.sum())
+    from paper_2211_14346_b200.binding import CHI2_DILEP_DTYPE
+    d = hepf.chi2_dilep(dev, idx_t, n, None, (160.0, 8)).cpu().numpy().reshape(-1).view(CHI2_DILEP_DTYPE)
+    torch.cuda.synchronize()
+    dref = hepf.chi2_dilep(dev0, idx_t0, n0, None, (160.0, 8)).cpu().numpy().reshape(-1).view(CHI2_DILEP_DTYPE)
+    assert np.array_equal(d["status"] == 2, dref["status"] == 2)             # applicability depends on the flags only
+    ok = d["status"] == 1
+    assert np.isfinite(d["chi2"][ok]).all() and np.isnan(d["chi2"][~ok]).all() and (d["jet_b"][~ok] == -1).all()
+    assert d[2000:].tobytes() == dref[2000:].tobytes()
 
 
 # ------------------------------------------------------------------------ derived per-event variables
