@@ -287,6 +287,25 @@ __device__ __forceinline__ bool certainly_no_real_root(double p, double q, doubl
   return delta > 1e-12 * mag && (p > 0.0 || w > 1e-12 * p2);
 }
 
+// Near-double pair of Q(t) = t^4 + p t^2 + q t + r next to t0 (Ferrari's pair discriminant vanished within rounding): the
+// critical point t* of Q there by Newton on Q', then the pair t* +- sqrt(-Q(t*) / (Q''(t*) / 2)) if Q(t*) and Q''(t*) have
+// opposite signs (the FP64 evaluation of Q resolves a tangency down to a few 1e-15 of sum |terms|; the closed form only to
+// about 1e-9 of its discriminant's terms).  Returns (larger, smaller), or NaNs if there is no real pair — an exact double root
+// included: the method skips those (R11c).
+__device__ __noinline__ double2 near_double_pair(double p, double q, double r, double t0) {
+  double t = t0;
+#pragma unroll 1
+  for (int it = 0; it < 4; it++) {
+    const double t2 = t * t, d1 = fma(fma(4.0, t2, 2.0 * p), t, q), d2 = fma(12.0, t2, 2.0 * p);
+    t -= d1 / d2;
+  }
+  const double t2 = t * t, Q = fma(t2, t2 + p, fma(q, t, r)), h = fma(6.0, t2, p);
+  const double ratio = -Q / h;
+  if (!(ratio > 0.0) || !(ratio < CUDART_INF)) return make_double2(CUDART_NAN, CUDART_NAN);
+  const double dl = sqrt(ratio);
+  return make_double2(t + dl, t - dl);
+}
+
 // Real roots of the depressed quartic by Ferrari's closed form, shifted back to x = t - aq; the polish happens later, on
 // the pair of conics.  Roots come out as pair A (xa[0], xa[1]) and pair B (xb[0], xb[1]).  Returns bit 0 = pair A real,
 // bit 1 = B.
@@ -307,8 +326,13 @@ __device__ __forceinline__ int ferrari(double p, double q, double r, double aq, 
     double is_; const double s = sqrt_rcp_fast(2.0 * m, is_), qs = q * is_;   // 2 qs' with qs' = q / (2 s); 1 / s comes with the root
     const double base = -2.0 * (m + p);
     const double dA = fma(-2.0, qs, base), dB = fma(2.0, qs, base);
-    if (dA >= 0.0) { const double sq = sqrt_fast(dA); xa[0] = fma(0.5, s + sq, -aq); xa[1] = fma(0.5, s - sq, -aq); mask |= 1; }
-    if (dB >= 0.0) { const double sq = sqrt_fast(dB); xb[0] = fma(0.5, sq - s, -aq); xb[1] = fma(-0.5, s + sq, -aq); mask |= 2; }
+    // A discriminant that vanishes within the rounding of its own terms is a near-double pair (almost tangent conics) whose
+    // existence the closed form cannot decide either way: the quartic itself can (out of line, a few solves per million)
+    const double marg = 0x1p-30 * fabs(base);      // base and 2 qs cancel in the vanishing discriminant, so |base| is the size of its terms
+    if (fabs(dA) < marg) { const double2 t = near_double_pair(p, q, r, 0.5 * s); if (t.x == t.x) { xa[0] = t.x - aq; xa[1] = t.y - aq; mask |= 1; } }
+    else if (dA >= 0.0) { const double sq = sqrt_fast(dA); xa[0] = fma(0.5, s + sq, -aq); xa[1] = fma(0.5, s - sq, -aq); mask |= 1; }
+    if (fabs(dB) < marg) { const double2 t = near_double_pair(p, q, r, -0.5 * s); if (t.x == t.x) { xb[0] = t.x - aq; xb[1] = t.y - aq; mask |= 2; } }
+    else if (dB >= 0.0) { const double sq = sqrt_fast(dB); xb[0] = fma(0.5, sq - s, -aq); xb[1] = fma(-0.5, s + sq, -aq); mask |= 2; }
   } else if (m == m) {               // q == 0 up to rounding: biquadratic t^4 + p t^2 + r (rare, out of line)
     const Biquad b = biquadratic_roots(p, r, aq);
     xa[0] = b.x[0]; xa[1] = b.x[1]; xb[0] = b.x[2]; xb[1] = b.x[3]; mask = b.mask;
