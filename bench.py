@@ -63,7 +63,9 @@ def search_kernel_name(V: int, nb6: bool) -> str:
     """The instantiation hepf_reconstruct_tth launches for V variations (hepf_reco.cu, reconstruct_impl): chunks of 32 variations
     (16 for n_b = 5, 6) unless that wastes more than an eighth of the last chunk's lanes, then 16 (8), and 8 for V <= 8."""
     waste32 = ((V + 31) & ~31) - V
-    if V <= 8:
+    if V <= 2:
+        vc4, vc6 = 1, 1
+    elif V <= 8:
         vc4, vc6 = 8, 8
     elif 8 * waste32 > V:
         vc4, vc6 = 16, 8

@@ -1170,7 +1170,8 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, con
   // chunk of variations per pass of the pipeline: 32 when that wastes at most an eighth of the lanes of the last chunk,
   // else 16 or 8.  32 (16 for n_b = 6) needs so much shared memory per warp that one block of 18 (19) warps fills an SM.
   const int waste32 = ((n_variations + 31) & ~31) - n_variations;
-  if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 2, 12, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
+  if (n_variations <= 2) rc = launch_search_both<1, 1, 2, 2, 10, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);   // lanes = pairings
+  else if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 2, 12, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
   else if (8 * waste32 > n_variations) rc = launch_search_both<16, 8, 2, 2, 10, 9>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
   else rc = launch_search_both<32, 16, 18, 19, 1, 1>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
   if (rc != HEPF_OK) return rc;
