@@ -25,16 +25,23 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
+def build(force: bool = False, verbose: bool = False, checked_out: str | None = None) -> str:
+    """Build libhepf.so in-tree.  checked_out = a path: build instead a CHECKED variant there (-DHEPF_CHECKED: every index into the
+    search kernel's hand-staged shared memory and into the workspace is tested and the kernel traps on a violation); used by
+    tests/test_checked_build.py, never by the product path."""
+    if checked_out is None and not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
-    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    bdir = os.path.join(HERE, "build") if checked_out is None else os.path.join(os.path.dirname(checked_out), "build_checked")
+    lib = LIB if checked_out is None else checked_out
+    os.makedirs(bdir, exist_ok=True)
     procs = []
     for s in SOURCES:
-        o = os.path.join(HERE, "build", s.replace(".cu", ".o"))
+        o = os.path.join(bdir, s.replace(".cu", ".o"))
         cmd = [nvcc, "-c", os.path.join(CSRC, s), "-o", o, "-I", os.path.join(ROOT, "include"), "-I", CSRC] + NVCC_FLAGS + EXTRA_FLAGS.get(s, [])
+        if checked_out is not None:
+            cmd.append("-DHEPF_CHECKED")
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(o)
     log = []
@@ -44,13 +51,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if p.returncode != 0:
             sys.stderr.write("\n".join(log))
             raise RuntimeError(f"nvcc failed on {s}")
-    subprocess.check_call([nvcc, "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a",
+    subprocess.check_call([nvcc, "-shared", "-o", lib] + objs + ["-gencode", "arch=compute_100a,code=sm_100a",
                                                                  "-cudart", "static"])
-    with open(os.path.join(HERE, "build", "ptxas.log"), "w") as f:
+    with open(os.path.join(bdir, "ptxas.log"), "w") as f:
         f.write("\n".join(log))
     if verbose:
         print("\n".join(log))
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

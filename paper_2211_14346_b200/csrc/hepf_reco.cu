@@ -32,6 +32,15 @@
 
 #include "hepf_common.cuh"
 
+// Checked build (build.py checked=True; tests/test_checked_build.py): every index into the per-warp queues and tables and into
+// the workspace is tested against its bound and the kernel traps on a violation.  compute-sanitizer is not available on the
+// pool this library is developed on; this is the stand-in for its memcheck on the one kernel that stages data by hand.
+#ifdef HEPF_CHECKED
+#define HEPF_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define HEPF_CHECK(cond) do { } while (0)
+#endif
+
 namespace hepf {
 
 constexpr int NBM = HEPF_MAX_B;   // candidate slots in the tables
@@ -619,9 +628,11 @@ struct __align__(16) WarpMem {
   };
   __device__ __forceinline__ double* sc() { return sc_; }
   __device__ __forceinline__ void push(int at, double x, uint32_t tag) {
+    HEPF_CHECK(at >= 0 && at < QCAP && tag <= TAG_MASK);
     q[at] = ((unsigned long long)__double_as_longlong(x) & ~(unsigned long long)TAG_MASK) | tag;
   }
   __device__ __forceinline__ void pop(int at, double& x, uint32_t& tag) const {
+    HEPF_CHECK(at >= 0 && at < QCAP);
     const unsigned long long en = q[at];
     x = __longlong_as_double((long long)(en & ~(unsigned long long)TAG_MASK)); tag = (uint32_t)en & TAG_MASK;   // tag bits cleared: x does not depend on its cell
   }
@@ -632,6 +643,7 @@ __device__ __forceinline__ void score_entry(const WarpMem<VC, NBT>& W, double x,
                                             double& best_ll, uint32_t& best_key) {
   const int vv = tag & 31, i = (tag >> 5) & 7, j = (tag >> 8) & 7, h = (tag >> 11) & 7, t = (tag >> 14) & 15, k = (tag >> 18) & 3;
   const int a1 = i * VC + vv, a2 = (NBT + j) * VC + vv;
+  HEPF_CHECK(vv < VC && i < NBT && j < NBT && i != j && t < (WarpMem<VC, NBT>::NP));
   const double2 abA = W.ab[i], abB = W.ab[NBT + j];
   const Conic A{abA.x, abA.y, W.cc[i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
   const Conic B{abB.x, abB.y, W.cc[NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
@@ -802,6 +814,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         if (keep) {
           const int at = sn + __popc(bk & lt);
           const double aqt = __hiloint2double(__double2hiint(qaq), (int)(((uint32_t)__double2loint(qaq) & ~STAG_MASK) | stag));
+          HEPF_CHECK(at >= 0 && at < SCAP && a1 < 2 * NBT * VC && a2 < 2 * NBT * VC && ap < NBT * (NBT - 1));
           W.s_pq[at] = make_double2(qp, qq); W.s_ra[at] = make_double2(qr, aqt);
         }
         sn += __popc(bk);
@@ -814,6 +827,7 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
           int mask = 0; uint32_t tag = 0;
           double xa[2], xb[2];
           if (lane < take) {
+            HEPF_CHECK(sn >= 0 && sn + lane < SCAP);
             const double2 pq = W.s_pq[sn + lane], ra = W.s_ra[sn + lane];
             const uint32_t st = (uint32_t)__double2loint(ra.y) & STAG_MASK;
             const double aq = __hiloint2double(__double2hiint(ra.y), (int)((uint32_t)__double2loint(ra.y) & ~STAG_MASK));   // tag bits cleared
@@ -901,6 +915,7 @@ reco_search_kernel(RecoCols ev, const uint32_t* __restrict__ idx, const int64_t*
       const int64_t k = g * epc + src;
       const EventHead h = load_head(ev, (int64_t)__ldg(idx + k));
       const uint32_t key = search_event<VC, NBT>(W, ev, h, V, k0, k1, P, lane);
+      HEPF_CHECK(k >= 0 && k < n_cap);
       if (lane == 0) winners[k] = make_uint2(key, key != 0xffffffffu ? 1u : 0u);
       // The nominal objects and the MET of the event, as this warp gathered them, go to the workspace as 42 columns of
       // n_cap doubles: the finalize kernel then reads them coalesced instead of gathering 40 scattered 64-byte DRAM atoms per
