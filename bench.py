@@ -113,7 +113,7 @@ def time_philox(hepf, n, steps, warmup):
     gbs = 8.0 * n / (ms * 1e-3) / 1e9
     return {"ms_per_step": ms, "value": n / (ms * 1e-3), "unit": "normals/s",
             "workload": f"cfg5: {n} normals, seed 7, counter 0",
-            "roofline": {"bound": "hbm", "kernel": "philox_normal_kernel<true>", "achieved": gbs, "peak": hbm, "unit": "GB/s",
+            "roofline": {"bound": "hbm", "kernel": "philox_normal_pairs_kernel", "achieved": gbs, "peak": hbm, "unit": "GB/s",
                          "frac": gbs / hbm, "traffic": None, "algorithmic_bytes": 8.0 * n, "kernel_ms": ms, "peak_source": src}}
 
 
