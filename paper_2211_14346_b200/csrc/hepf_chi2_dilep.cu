@@ -78,7 +78,7 @@ __device__ __forceinline__ LegMin leg_min(const Q4& l, const Q4 (&b)[4], int nbt
 
 __device__ __forceinline__ double grid_u(int g, double gn) { return (double)(2 * g + 1) / gn - 1.0; }
 
-__global__ void __launch_bounds__(32 * CD_WARPS)
+__global__ void __launch_bounds__(32 * CD_WARPS, 5)   // 96 registers, 20 warps per SM: the dependent FP64 chains want the occupancy (164 registers unbounded: 11.3 vs 9.5 ms)
 chi2_dilep_kernel(DilepCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, hepf_chi2_params_t P, double split_range,
                   int G, hepf_chi2_dilep_t* __restrict__ out) {
   const int lane = threadIdx.x & 31;
