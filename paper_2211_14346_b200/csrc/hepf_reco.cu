@@ -729,7 +729,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         }
       }
     }
-    if (FUSE_M && vok) { W.M[vv] = __dadd_rn(W.met[0], -ax); W.M[VC + vv] = __dadd_rn(W.met[1], -ay); }
+    const double Mx_own = __dadd_rn(W.met[0], -ax), My_own = __dadd_rn(W.met[1], -ay);   // (only meaningful with FUSE_M)
+    if (FUSE_M && vok) { W.M[vv] = Mx_own; W.M[VC + vv] = My_own; }
     __syncwarp();
     if (v0 == 0 && lane < n_ord) {     // pair constants of every ordered pairing: once per event
       const int i = (lane * dmul) >> dsh; int j = lane - i * (nb - 1); j += (j >= i);
@@ -748,7 +749,62 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       }
     }
     if (!FUSE_M) __syncwarp();
-    // ---- B: leg conics (leg 0: l+ with candidate c; leg 1: l- with candidate c, shifted by MET') -------------------------
+    // ---- B: leg conics (leg 0: l+ with candidate c; leg 1: l- with candidate c, shifted by MET').  With 32-variation chunks a
+    //      lane owns a variation: its scales and their reciprocals are loaded once (6 reciprocals instead of 16), the eight
+    //      conics are unrolled with compile-time table offsets, and MET' is the lane's own from stage A.
+    double sv[4] = {1.0, 1.0, 1.0, 1.0};        // the lane's scales of the four candidates (32-variation chunks: a lane owns a variation)
+    if (NBT == 4 && LPB == 1) {
+      if (vok) {
+        double rv[4];
+#pragma unroll
+        for (int c = 0; c < 4; c++) { sv[c] = W.sc()[(2 + ((h.cand >> (4 * c)) & 15)) * VC + vv]; rv[c] = rcp_fast(sv[c]); }
+#pragma unroll
+        for (int leg = 0; leg < 2; leg++) {
+          const int ls = leg ? 1 - h.lp_slot : h.lp_slot;
+          const double sl = W.sc()[ls * VC + vv], rl = rcp_fast(sl);
+#pragma unroll
+          for (int c = 0; c < 4; c++) {
+            const int fi = leg * NBT + c;
+            Frame F;
+            F.a = W.ab[fi].x; F.b = W.ab[fi].y; F.c = W.cc[fi]; F.c1 = W.frb[0][fi]; F.c2 = W.frb[1][fi];
+            F.d1 = W.frb[2][fi]; F.d2 = W.frb[3][fi]; F.g1 = W.frb[4][fi]; F.g2 = W.frb[5][fi]; F.h1 = W.frb[6][fi];
+            F.ile = W.frb[7][fi]; F.hml2 = W.frb[8][fi]; F.hmb2 = W.frb[9][fi]; F.bln = W.frb[10][fi];
+            Conic q; double c0_;
+            q.a = F.a; q.b = F.b; q.c = F.c;
+            conic_def(F, sl, sv[c], rl, rv[c], hmw2, hcm, c0_, q.d, q.e, q.f);
+            if (leg) q = shift_conic(q, Mx_own, My_own);
+            const int at = fi * VC + vv;
+            W.def[0][at] = q.d; W.def[1][at] = q.e; W.def[2][at] = q.f;
+          }
+        }
+      }
+    } else
+    if (NBT == 4 && LPB == 2) {         // 16-variation chunks: a lane owns a (variation, leg): one lepton scale and reciprocal, the four
+                                        // candidates unrolled (for n_b = 6 the rolled loop below is the faster one: measured)
+      if (vok) {
+        const int leg = sub;
+        const int ls = leg ? 1 - h.lp_slot : h.lp_slot;
+        const double sl = W.sc()[ls * VC + vv], rl = rcp_fast(sl);
+        const double Mx = W.M[vv], My = W.M[VC + vv];
+#pragma unroll
+        for (int c = 0; c < NBT; c++) {
+          if (c < nb) {
+            const int fi = leg * NBT + c;
+            const double sb = W.sc()[(2 + ((h.cand >> (4 * c)) & 15)) * VC + vv];
+            Frame F;
+            F.a = W.ab[fi].x; F.b = W.ab[fi].y; F.c = W.cc[fi]; F.c1 = W.frb[0][fi]; F.c2 = W.frb[1][fi];
+            F.d1 = W.frb[2][fi]; F.d2 = W.frb[3][fi]; F.g1 = W.frb[4][fi]; F.g2 = W.frb[5][fi]; F.h1 = W.frb[6][fi];
+            F.ile = W.frb[7][fi]; F.hml2 = W.frb[8][fi]; F.hmb2 = W.frb[9][fi]; F.bln = W.frb[10][fi];
+            Conic q; double c0_;
+            q.a = F.a; q.b = F.b; q.c = F.c;
+            conic_def(F, sl, sb, rl, rcp_fast(sb), hmw2, hcm, c0_, q.d, q.e, q.f);
+            if (leg) q = shift_conic(q, Mx, My);
+            const int at = fi * VC + vv;
+            W.def[0][at] = q.d; W.def[1][at] = q.e; W.def[2][at] = q.f;
+          }
+        }
+      }
+    } else
 #pragma unroll 1
     for (int c0 = 0; c0 < 2 * nb; c0 += LPB) {
       const int comb = c0 + sub;
@@ -770,6 +826,22 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
       }
     }
     // ---- H: Higgs term of every unordered candidate pair ---------------------------------------------------------------
+    if (NBT == 4 && LPB == 1) {         // a lane owns a variation: the six pairs unrolled, on the scales stage B loaded
+      if (vok) {
+        double sq[4];
+#pragma unroll
+        for (int c = 0; c < 4; c++) sq[c] = sv[c] * sv[c];
+        int pi = 0;
+#pragma unroll
+        for (int kk = 0; kk < 4; kk++)
+#pragma unroll
+          for (int ll = kk + 1; ll < 4; ll++, pi++) {
+            const double m2 = fma(sq[kk], W.hm2[kk], fma(sq[ll], W.hm2[ll], (sv[kk] * sv[ll]) * W.hdot[pi]));
+            const double t = (sqrt_fast(m2 < 0.0 ? 0.0 : m2) - P.m_higgs) * inv_sh;
+            W.ht[pi * VC + vv] = -0.5 * (t * t);
+          }
+      }
+    } else
 #pragma unroll 1
     for (int p0 = 0; p0 < n_pair; p0 += LPB) {
       const int p = p0 + sub;
