@@ -70,7 +70,7 @@ extern "C" double hepf_timing_ms(int from_slot, int to_slot) {
   return (double)ms;
 }
 extern "C" const char* hepf_last_error(void) { return g_err; }
-extern "C" const char* hepf_version(void) { return "hepf 0.2 (sm_100a)"; }
+extern "C" const char* hepf_version(void) { return "hepf 0.3 (sm_100a)"; }
 extern "C" int64_t hepf_launch_count(int reset) {
   int64_t v = g_launches;
   if (reset) g_launches = 0;
