@@ -376,19 +376,26 @@ __device__ __forceinline__ void newton_xy(const Conic& A, const Conic& B, double
     x -= dx; y -= dy; mv = m;
   }
 }
-__device__ __noinline__ double2 refine_more(const Conic A, const Conic B, double x, double y) {
+// reject: a point that has not settled after these steps (the last one still moved it by more than 1e-6) is not a solution —
+// at an exactly tangent pair of conics Newton wanders instead of converging and the likelihood of where it happens to stand
+// means nothing — and is returned as NaN, which never wins the argmax.  The search rejects; the finalize kernel, which only
+// re-derives a winner the search has accepted, does not.
+__device__ __noinline__ double2 refine_more(const Conic A, const Conic B, double x, double y, bool reject) {
+  double mv = 0.0;
 #pragma unroll 1
   for (int it = 0; it < 6; it++) {
-    double mv = 0.0;
+    mv = 0.0;
     newton_xy<true>(A, B, x, y, mv);
     if (mv <= 1e-10 * (fabs(x) + fabs(y))) break;
   }
+  if (reject && !(mv <= 1e-6 * (fabs(x) + fabs(y)))) return make_double2(CUDART_NAN, CUDART_NAN);
   return make_double2(x, y);
 }
 
 // One intersection: start from the Ferrari root x and y = -D1/D2, then two Newton steps on the pair of conics in
 // (x, y).  The quotient alone cancels when D2(x) is small; the 2x2 system is conditioned like the intersection
 // itself (R11a).
+template <bool REJECT>
 __device__ __forceinline__ void refine_xy(const Conic& A, const Conic& B, double& x, double& y) {
   const Lines L = lines_of(A, B);
   // D2(x) = 0 means the two conics share both y at this x: a double root in x, which the method skips (R11c);
@@ -402,7 +409,7 @@ __device__ __forceinline__ void refine_xy(const Conic& A, const Conic& B, double
   if (mv > 1e-6 * (fabs(x) + fabs(y))) newton_xy<false>(A, B, x, y, mv); else mv = 0.0;
   // a second step that still moved the point by more than 1e-10 (relative) means near-tangent conics (linear
   // convergence): keep polishing out of line, up to six more steps
-  if (mv > 1e-10 * (fabs(x) + fabs(y))) { const double2 r = refine_more(A, B, x, y); x = r.x; y = r.y; }
+  if (mv > 1e-10 * (fabs(x) + fabs(y))) { const double2 r = refine_more(A, B, x, y, REJECT); x = r.x; y = r.y; }
 }
 
 // log-likelihood of one refined root (Higgs term ht already chosen)
@@ -648,7 +655,7 @@ __device__ __forceinline__ void score_entry(const WarpMem<VC, NBT>& W, double x,
   const Conic A{abA.x, abA.y, W.cc[i], W.def[0][a1], W.def[1][a1], W.def[2][a1]};
   const Conic B{abB.x, abB.y, W.cc[NBT + j], W.def[0][a2], W.def[1][a2], W.def[2][a2]};
   double y;
-  refine_xy(A, B, x, y);
+  refine_xy<true>(A, B, x, y);
   const double ll = loglik_of(x, y, W.M[vv], W.M[VC + vv], W.ht[t * VC + vv], inv_lambda);
   if (ll >= best_ll) {               // the key is only needed by a candidate that can replace the incumbent (rare per lane)
     const uint32_t key = make_key(v0 + vv, i, j, h, k);
@@ -1064,7 +1071,7 @@ __device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_
   double xs[4], ys[4]; int nr = 0;
   if (mask & 1) { xs[0] = xa[0]; xs[1] = xa[1]; nr = 2; }
   if (mask & 2) { xs[nr] = xb[0]; xs[nr + 1] = xb[1]; nr += 2; }
-  for (int r = 0; r < nr; r++) refine_xy(A, B, xs[r], ys[r]);
+  for (int r = 0; r < nr; r++) refine_xy<false>(A, B, xs[r], ys[r]);
   const int rs = ksel < nr ? ksel : 0;
   const double xx = nr ? xs[rs] : CUDART_NAN, yy = nr ? ys[rs] : CUDART_NAN;
   int rank = 0;

@@ -758,3 +758,24 @@ def test_chi2_dilep_parity(hepf):
     for bad in ((160.0, 0), (160.0, 65), (-1.0, 8)):
         with pytest.raises(hepf.HepfError):
             hepf.chi2_dilep(dev, idx_t, 8, None, bad)
+
+
+def test_regression_events_at_tangent_conics(hepf):
+    """Two events that full-size parity runs of this build found.  cfg4 event 19 836 077: the winning pair of
+    roots is 7e-6 apart (tangency measure 2.9e-12) — Ferrari's pair discriminant cannot decide it, the quartic itself can
+    (near_double_pair).  cfg3 event 587 363: at variation 195 one pairing has conics that are tangent to 3e-18; Newton on the
+    pair wanders there and the likelihood of an unsettled point once beat the true winner (variation 171) — the search now
+    rejects refinements that have not settled."""
+    import torch
+    for cid, e0 in ((4, 19_836_077), (3, 587_363)):
+        cfg = hs.CONFIGS[cid]
+        st = cfg.events(4, first_event=e0)
+        assert st.event_base == e0
+        dev = hepf.DeviceEvents.from_host(st)
+        idx = np.zeros(1, dtype=np.uint32)
+        idx_t = torch.zeros(1, dtype=torch.int32, device="cuda")
+        got = _gpu_reco(hepf, dev, idx_t, 1, cfg.n_variations, cfg.reco_seed)
+        want, aux = oracle.reconstruct_tth(st, idx, cfg.n_variations, cfg.reco_seed)
+        cls = assert_parity(st, got, want, aux, cfg.n_variations, cfg.reco_seed, max_excused_frac=0.0, label=f"cfg{cid} event {e0}")
+        assert cls["match"] + cls["oracle_far"] == 1
+        assert all(int(got[0][f]) == int(want[0][f]) for f in ("variation", "jet_b", "jet_bbar", "jet_h1", "jet_h2", "root"))
