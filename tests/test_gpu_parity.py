@@ -779,3 +779,50 @@ def test_regression_events_at_tangent_conics(hepf):
         cls = assert_parity(st, got, want, aux, cfg.n_variations, cfg.reco_seed, max_excused_frac=0.0, label=f"cfg{cid} event {e0}")
         assert cls["match"] + cls["oracle_far"] == 1
         assert all(int(got[0][f]) == int(want[0][f]) for f in ("variation", "jet_b", "jet_bbar", "jet_h1", "jet_h2", "root"))
+
+
+def test_select_and_reconstruct_are_capturable_in_a_cuda_graph(hepf):
+    """Every device entry point only enqueues on the caller's stream and nothing comes back to the host between hepf_select and
+    hepf_reconstruct_tth_n (the list length stays on the device), so the whole path can be captured once in a CUDA graph and
+    replayed — the remedy for launch-bound small samples (cfg1: six launches for 0.05 ms of work).  The replay gives the bytes
+    of the direct calls."""
+    import torch
+    cfg = hs.CONFIGS[1]
+    st = cfg.events()
+    dev = hepf.DeviceEvents.from_host(st)
+    n, V = st.n_events, cfg.n_variations
+    L = hepf.load()
+    out_idx = torch.empty(n, dtype=torch.int32, device="cuda"); out_count = torch.zeros(1, dtype=torch.int64, device="cuda")
+    out_cf = torch.zeros(32, dtype=torch.int64, device="cuda")
+    ws = torch.empty(int(L.hepf_select_workspace_bytes(n)) + 256, dtype=torch.uint8, device="cuda")
+    out_best = torch.zeros((n, 128), dtype=torch.uint8, device="cuda")
+    reco_ws = torch.empty(int(L.hepf_reconstruct_workspace_bytes(n, V)) + 256, dtype=torch.uint8, device="cuda")
+
+    def path(stream):
+        hepf.select(dev, cfg.cuts, out_idx=out_idx, out_count=out_count, out_cutflow=out_cf, ws=ws, stream=stream)
+        hepf.reconstruct_tth_n(dev, out_idx, out_count, n, V, cfg.reco_seed, None, out_best=out_best, ws=reco_ws, stream=stream)
+
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        path(s)                                   # warm-up: function attributes and occupancy are looked up once per thread
+    torch.cuda.synchronize()
+    m = int(out_count.item())
+    direct = out_best[:m].cpu().numpy().copy(); direct_idx = out_idx[:m].cpu().numpy().copy()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        path(torch.cuda.current_stream())
+    for _ in range(3):
+        out_best.zero_(); out_count.zero_(); out_idx.zero_()
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        assert int(out_count.item()) == m and np.array_equal(out_idx[:m].cpu().numpy(), direct_idx)
+        assert out_best[:m].cpu().numpy().tobytes() == direct.tobytes()
+    # device time of a replay against the six direct launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); [g.replay() for _ in range(50)]; e1.record(); torch.cuda.synchronize()
+    t_graph = e0.elapsed_time(e1) / 50
+    cur = torch.cuda.current_stream()
+    e0.record(); [path(cur) for _ in range(50)]; e1.record(); torch.cuda.synchronize()
+    t_direct = e0.elapsed_time(e1) / 50
+    print(f"[graph] cfg1 step: {t_direct * 1e3:.1f} us direct, {t_graph * 1e3:.1f} us as a graph replay")
