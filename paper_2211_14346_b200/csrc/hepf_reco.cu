@@ -611,6 +611,7 @@ struct __align__(16) WarpMem {
   double ht[VC * NP];            // Higgs term of candidate pair (k, l), k < l
   double hm2[NBT];               // per event: nominal m^2 of candidate c
   double hdot[NP];               // per event: 2 (b_k . b_l) of the nominal candidates k < l (Minkowski product)
+  uint32_t hp[NP + (NP & 1)];    // per event: the p-th pair as k | l << 4 | object of k << 8 | object of l << 12 | table row << 16
   double M[VC * 2];              // MET'
   double obj[10 * 4];            // nominal (px, py, pz, E)
   double ks[10];                 // kappa * sigma
@@ -690,6 +691,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
     const double* bk = &W.obj[(2 + ((h.cand >> (4 * kk)) & 15)) * 4];
     const double* bl = &W.obj[(2 + ((h.cand >> (4 * ll)) & 15)) * 4];
     W.hdot[pair_index<NBT>(kk, ll)] = 2.0 * fma(bk[3], bl[3], -fma(bk[0], bl[0], fma(bk[1], bl[1], bk[2] * bl[2])));
+    W.hp[lane] = (uint32_t)kk | ((uint32_t)ll << 4) | ((2u + ((h.cand >> (4 * kk)) & 15u)) << 8) | ((2u + ((h.cand >> (4 * ll)) & 15u)) << 12) |
+                 ((uint32_t)pair_index<NBT>(kk, ll) << 16);
   } else if (lane >= 16 && lane < 16 + nb) {
     const double* b = &W.obj[(2 + ((h.cand >> (4 * (lane - 16))) & 15)) * 4];
     W.hm2[lane - 16] = fma(b[3], b[3], -fma(b[0], b[0], fma(b[1], b[1], b[2] * b[2])));
@@ -812,6 +815,29 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
         }
       }
     } else
+    if (NBT == 6 && LPB == 2) {         // a lane owns a (variation, leg): lepton scale and reciprocal hoisted, candidates in a rolled loop
+      if (vok) {
+        const int leg = sub;
+        const int ls = leg ? 1 - h.lp_slot : h.lp_slot;
+        const double sl = W.sc()[ls * VC + vv], rl = rcp_fast(sl);
+        const double Mx = W.M[vv], My = W.M[VC + vv];
+#pragma unroll 1
+        for (int c = 0; c < nb; c++) {
+          const int fi = leg * NBT + c;
+          const double sb = W.sc()[(2 + ((h.cand >> (4 * c)) & 15)) * VC + vv];
+          Frame F;
+          F.a = W.ab[fi].x; F.b = W.ab[fi].y; F.c = W.cc[fi]; F.c1 = W.frb[0][fi]; F.c2 = W.frb[1][fi];
+          F.d1 = W.frb[2][fi]; F.d2 = W.frb[3][fi]; F.g1 = W.frb[4][fi]; F.g2 = W.frb[5][fi]; F.h1 = W.frb[6][fi];
+          F.ile = W.frb[7][fi]; F.hml2 = W.frb[8][fi]; F.hmb2 = W.frb[9][fi]; F.bln = W.frb[10][fi];
+          Conic q; double c0_;
+          q.a = F.a; q.b = F.b; q.c = F.c;
+          conic_def(F, sl, sb, rl, rcp_fast(sb), hmw2, hcm, c0_, q.d, q.e, q.f);
+          if (leg) q = shift_conic(q, Mx, My);
+          const int at = fi * VC + vv;
+          W.def[0][at] = q.d; W.def[1][at] = q.e; W.def[2][at] = q.f;
+        }
+      }
+    } else
 #pragma unroll 1
     for (int c0 = 0; c0 < 2 * nb; c0 += LPB) {
       const int comb = c0 + sub;
@@ -853,9 +879,8 @@ __device__ __forceinline__ uint32_t search_event(WarpMem<VC, NBT>& W, const Reco
     for (int p0 = 0; p0 < n_pair; p0 += LPB) {
       const int p = p0 + sub;
       if (vok && p < n_pair) {
-        const int kk = (int)(PK >> (4 * p)) & 15, ll = (int)(PL >> (4 * p)) & 15;
-        const int j1 = 2 + ((h.cand >> (4 * kk)) & 15), j2 = 2 + ((h.cand >> (4 * ll)) & 15);
-        const int pi = pair_index<NBT>(kk, ll);
+        const uint32_t hd = W.hp[p];
+        const int kk = hd & 15, ll = (hd >> 4) & 15, j1 = (hd >> 8) & 15, j2 = (hd >> 12) & 15, pi = hd >> 16;
         const double sk = W.sc()[j1 * VC + vv], sl = W.sc()[j2 * VC + vv];
         const double m2 = fma(sk * sk, W.hm2[kk], fma(sl * sl, W.hm2[ll], (sk * sl) * W.hdot[pi]));
         // a NaN (garbage inputs: inf - inf) stays a NaN, so that such a pair never wins here while the finalize kernel, which
