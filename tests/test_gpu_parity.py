@@ -473,20 +473,31 @@ def test_histogram_counts_are_bit_exact(hepf):
 
 
 # ------------------------------------------------------------------------------------- chi^2 (semileptonic ttbar)
+def _chi2_tol(pz):
+    """1e-9 relative (north_star), unless the conditioning of the problem itself is worse: the masses are
+    recomputed from four-vectors, m^2 = E^2 - |p|^2 cancels by (E / m)^2, and the p_z that solves m(l nu) = m_W inherits
+    it; with a p_z beyond about 15 TeV (events in 10^6, and not a physical neutrino) BOTH sides carry more than 1e-9 of
+    rounding noise, about 256 eps (p_z / m_W)^2."""
+    return np.maximum(1e-9, 256 * 2.0 ** -53 * (np.abs(pz) / 80.4) ** 2)
+
+
 def _chi2_compare(got, want, second):
     assert np.array_equal(got["event"], want["event"]) and np.array_equal(got["status"], want["status"])
     assert np.array_equal(got["n_comb"], want["n_comb"])
     ok = want["status"] == 1
     assert np.isnan(got["chi2"][~ok]).all() and (got["jet_b_lep"][~ok] == -1).all()
+    tol = _chi2_tol(want["nu_pz"][ok])
     rel = np.abs(got["chi2"][ok] - want["chi2"][ok]) / np.maximum(1.0, np.abs(want["chi2"][ok]))
-    assert rel.max() <= 1e-9
+    assert (rel <= tol).all()
     keys = ("jet_b_lep", "jet_b_had", "jet_q1", "jet_q2", "solution")
     same = np.all([got[k][ok] == want[k][ok] for k in keys], axis=0)
     tie = (second[ok] - want["chi2"][ok]) <= 1e-9 * np.maximum(1.0, np.abs(want["chi2"][ok]))   # north_star's near-tie rule
     assert (same | tie).all()
     for f in ("nu_pz", "m_top_lep", "m_top_had", "m_w_lep", "m_w_had"):
         g, w = got[f][ok][same], want[f][ok][same]
-        assert (np.abs(g - w) <= 1e-9 * np.maximum(1.0, np.abs(w))).all(), f
+        assert np.array_equal(np.isnan(g), np.isnan(w)), f          # single top: the absent top's fields are NaN on both sides
+        fin = ~np.isnan(w)
+        assert (np.abs(g[fin] - w[fin]) <= tol[same][fin] * np.maximum(1.0, np.abs(w[fin]))).all(), f
     return int(same.sum()), int(ok.sum())
 
 
@@ -688,23 +699,12 @@ def test_chi2_single_top_parity(hepf):
         for par in (None, (170.0, 81.0, 9.0, 6.0)):
             got = hepf.chi2_single_top(dev, idx_t, len(idx), mode, par).cpu().numpy().reshape(-1).view(CHI2_DTYPE)
             want, second = oracle.chi2_single_top(st, idx, mode, par)
-            assert np.array_equal(got["event"], want["event"]) and np.array_equal(got["status"], want["status"])
-            assert np.array_equal(got["n_comb"], want["n_comb"])
             ok = want["status"] == 1
-            assert 0.5 < ok.mean() < 0.9 and np.isnan(got["chi2"][~ok]).all()
-            rel = np.abs(got["chi2"][ok] - want["chi2"][ok]) / np.maximum(1.0, np.abs(want["chi2"][ok]))
-            assert rel.max() <= 1e-9
-            keys = ("jet_b_lep", "jet_b_had", "jet_q1", "jet_q2", "solution")
-            same = np.all([got[k][ok] == want[k][ok] for k in keys], axis=0)
-            tie = (second[ok] - want["chi2"][ok]) <= 1e-9 * np.maximum(1.0, np.abs(want["chi2"][ok]))
+            assert 0.5 < ok.mean() < 0.9
             # Wt with a hadronic top: both p_z solutions satisfy m(l nu) = m_W, the leptonic W term is 0 for both and the chi^2 an
             # exact tie between them (north_star's near-tie rule): the solution index is then arbitrary, everything else is not
-            assert (same | tie).all() and same.mean() > (0.999 if mode == 1 else 0.8)
-            for f in ("nu_pz", "m_top_lep", "m_top_had", "m_w_lep", "m_w_had"):
-                g, w = got[f][ok][same], want[f][ok][same]
-                assert np.array_equal(np.isnan(g), np.isnan(w)), f
-                fin = ~np.isnan(w)
-                assert (np.abs(g[fin] - w[fin]) <= 1e-9 * np.maximum(1.0, np.abs(w[fin]))).all(), f
+            same, n_ok = _chi2_compare(got, want, second)
+            assert n_ok == ok.sum() and same / n_ok > (0.999 if mode == 1 else 0.8)
     with pytest.raises(hepf.HepfError):
         hepf.chi2_single_top(dev, idx_t, 5, 0)
 
@@ -726,16 +726,17 @@ def test_chi2_dilep_parity(hepf):
         dead = ~ok
         assert np.isnan(got["chi2"][dead]).all() and (got["jet_b"][dead] == -1).all() and (got["grid_x"][dead] == -1).all()
         g, w = got[ok], want[ok]
-        assert np.all(np.abs(g["chi2"] - w["chi2"]) <= 1e-9 * np.maximum(1.0, w["chi2"]))
+        tol = _chi2_tol(np.maximum(np.abs(w["nu"][:, 2]), np.abs(w["nubar"][:, 2])))
+        assert np.all(np.abs(g["chi2"] - w["chi2"]) <= tol * np.maximum(1.0, w["chi2"]))
         tie = second[ok] <= w["chi2"] * (1 + 1e-9) + 1e-12
         keys = ("jet_b", "jet_bbar", "grid_x", "grid_y", "sol_nu", "sol_nubar")
         same = np.all([g[f] == w[f] for f in keys], axis=0)
         assert (same | tie).all(), np.flatnonzero(~(same | tie))[:5]
         for f in ("nu", "nubar"):
             sc = np.maximum(1.0, np.abs(w[f]).max(axis=1))
-            assert np.all(np.abs(g[f][same] - w[f][same]).max(axis=1) <= 1e-9 * sc[same])
+            assert np.all(np.abs(g[f][same] - w[f][same]).max(axis=1) <= tol[same] * sc[same])
         for f in ("m_top", "m_antitop", "m_wplus", "m_wminus"):
-            assert np.all(np.abs(g[f][same] - w[f][same]) <= 1e-9 * np.maximum(1.0, w[f][same]))
+            assert np.all(np.abs(g[f][same] - w[f][same]) <= tol[same] * np.maximum(1.0, w[f][same]))
         return int(ok.sum()), int(same.sum())
 
     st = hs.generate(1500, 51, with_truth=False)
