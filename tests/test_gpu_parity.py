@@ -709,36 +709,38 @@ def test_chi2_single_top_parity(hepf):
         hepf.chi2_single_top(dev, idx_t, 5, 0)
 
 
+def _chi2_dilep_compare(hepf, st, idx, par=None, split=None):
+    import torch
+    from paper_2211_14346_b200.binding import CHI2_DILEP_DTYPE
+    dev = hepf.DeviceEvents.from_host(st)
+    idx_t = torch.from_numpy(np.ascontiguousarray(idx, dtype=np.uint32).view(np.int32)).cuda()
+    got = hepf.chi2_dilep(dev, idx_t, len(idx), par, split).cpu().numpy().reshape(-1).view(CHI2_DILEP_DTYPE)
+    want, second = oracle.chi2_dilep(st, idx, par, split, n_threads=16)
+    assert np.array_equal(got["status"], want["status"]) and np.array_equal(got["event"], want["event"])
+    assert np.array_equal(got["n_comb"], want["n_comb"])
+    ok = want["status"] == 1
+    dead = ~ok
+    assert np.isnan(got["chi2"][dead]).all() and (got["jet_b"][dead] == -1).all() and (got["grid_x"][dead] == -1).all()
+    g, w = got[ok], want[ok]
+    tol = _chi2_tol(np.maximum(np.abs(w["nu"][:, 2]), np.abs(w["nubar"][:, 2])))
+    assert np.all(np.abs(g["chi2"] - w["chi2"]) <= tol * np.maximum(1.0, w["chi2"]))
+    tie = second[ok] <= w["chi2"] * (1 + 1e-9) + 1e-12
+    keys = ("jet_b", "jet_bbar", "grid_x", "grid_y", "sol_nu", "sol_nubar")
+    same = np.all([g[f] == w[f] for f in keys], axis=0)
+    assert (same | tie).all(), np.flatnonzero(~(same | tie))[:5]
+    for f in ("nu", "nubar"):
+        sc = np.maximum(1.0, np.abs(w[f]).max(axis=1))
+        assert np.all(np.abs(g[f][same] - w[f][same]).max(axis=1) <= tol[same] * sc[same])
+    for f in ("m_top", "m_antitop", "m_wplus", "m_wminus"):
+        assert np.all(np.abs(g[f][same] - w[f][same]) <= tol[same] * np.maximum(1.0, w[f][same]))
+    return int(ok.sum()), int(same.sum())
+
+
 def test_chi2_dilep_parity(hepf):
     """hepf_chi2_dilep (eq. 1, dileptonic; R15) against oracle/oracle_chi2_dilep.cpp: status,
     n_comb and (outside near-ties of the oracle's two best values) every index exactly, chi^2 / momenta / masses to 1e-9."""
     import torch
-    from paper_2211_14346_b200.binding import CHI2_DILEP_DTYPE
-
-    def run(st, idx, par=None, split=None):
-        dev = hepf.DeviceEvents.from_host(st)
-        idx_t = torch.from_numpy(np.ascontiguousarray(idx, dtype=np.uint32).view(np.int32)).cuda()
-        got = hepf.chi2_dilep(dev, idx_t, len(idx), par, split).cpu().numpy().reshape(-1).view(CHI2_DILEP_DTYPE)
-        want, second = oracle.chi2_dilep(st, idx, par, split, n_threads=16)
-        assert np.array_equal(got["status"], want["status"]) and np.array_equal(got["event"], want["event"])
-        assert np.array_equal(got["n_comb"], want["n_comb"])
-        ok = want["status"] == 1
-        dead = ~ok
-        assert np.isnan(got["chi2"][dead]).all() and (got["jet_b"][dead] == -1).all() and (got["grid_x"][dead] == -1).all()
-        g, w = got[ok], want[ok]
-        tol = _chi2_tol(np.maximum(np.abs(w["nu"][:, 2]), np.abs(w["nubar"][:, 2])))
-        assert np.all(np.abs(g["chi2"] - w["chi2"]) <= tol * np.maximum(1.0, w["chi2"]))
-        tie = second[ok] <= w["chi2"] * (1 + 1e-9) + 1e-12
-        keys = ("jet_b", "jet_bbar", "grid_x", "grid_y", "sol_nu", "sol_nubar")
-        same = np.all([g[f] == w[f] for f in keys], axis=0)
-        assert (same | tie).all(), np.flatnonzero(~(same | tie))[:5]
-        for f in ("nu", "nubar"):
-            sc = np.maximum(1.0, np.abs(w[f]).max(axis=1))
-            assert np.all(np.abs(g[f][same] - w[f][same]).max(axis=1) <= tol[same] * sc[same])
-        for f in ("m_top", "m_antitop", "m_wplus", "m_wminus"):
-            assert np.all(np.abs(g[f][same] - w[f][same]) <= tol[same] * np.maximum(1.0, w[f][same]))
-        return int(ok.sum()), int(same.sum())
-
+    run = lambda *a: _chi2_dilep_compare(hepf, *a)   # noqa: E731
     st = hs.generate(1500, 51, with_truth=False)
     n_ok, n_same = run(st, np.arange(1500))
     assert n_ok == 1500 and n_same >= n_ok - 2
@@ -759,6 +761,31 @@ def test_chi2_dilep_parity(hepf):
     for bad in ((160.0, 0), (160.0, 65), (-1.0, 8)):
         with pytest.raises(hepf.HepfError):
             hepf.chi2_dilep(dev, idx_t, 8, None, bad)
+
+
+def test_chi2_soak_a_million_events_per_mode(hepf):
+    """Every chi^2 entry point on samples large enough to meet the rare cases: 10^6 semileptonic events through
+    hepf_chi2_semilep and both single-top modes, 10^5 + 3 10^5 dileptonic events through hepf_chi2_dilep; same gate as the
+    parity tests.  These seeds contain the three events whose |p_z| of tens to hundreds of TeV puts oracle and kernel
+    1.1 - 1.5e-9 apart (the conditioning bound of _chi2_tol), which the smaller samples above do not reach."""
+    import torch
+    from paper_2211_14346_b200.binding import CHI2_DTYPE
+    st = hs.generate(1_000_000, 4242, semilep=True, with_truth=False)
+    dev = hepf.DeviceEvents.from_host(st); n = st.n_events
+    idx = np.arange(n, dtype=np.uint32); idx_t = torch.from_numpy(idx.view(np.int32)).cuda()
+    got = hepf.chi2_semilep(dev, idx_t, n).cpu().numpy().reshape(-1).view(CHI2_DTYPE)
+    want, second = oracle.chi2_semilep(st, idx)
+    same, ok = _chi2_compare(got, want, second)
+    assert ok == n and same >= ok - 10
+    for mode in (1, 2):
+        got = hepf.chi2_single_top(dev, idx_t, n, mode).cpu().numpy().reshape(-1).view(CHI2_DTYPE)
+        want, second = oracle.chi2_single_top(st, idx, mode)
+        same, ok = _chi2_compare(got, want, second)
+        assert ok == n and same >= (ok - 10 if mode == 1 else 0.8 * ok)
+    del dev
+    for seed, n in ((4343, 100_000), (4344, 300_000)):
+        n_ok, n_same = _chi2_dilep_compare(hepf, hs.generate(n, seed, with_truth=False), np.arange(n))
+        assert n_ok == n and n_same >= n_ok - 20
 
 
 def test_regression_events_at_tangent_conics(hepf):
