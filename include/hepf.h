@@ -150,6 +150,26 @@ int hepf_select_planned(const hepf_events_t* events, const hepf_cut_t* host_cuts
 size_t hepf_select_planned_workspace_bytes(int64_t n_events);
 
 /*
+ * hepf_select_static — hepf_select (§4 :136) for callers that cannot allocate device memory
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): same arguments, same kernels and
+ * byte-identical results, but no workspace argument.  The per-warp pass masks and the per-block survivor counts live in
+ * a file-scope device array of the library, HEPF_SELECT_STATIC_BYTES (about 0.5 MB) on EVERY GPU that loads the library,
+ * held until the process exits.  The call allocates nothing: no cudaMalloc / cudaFree and no allocating library routine;
+ * its first call on a device looks the array's device address up (cudaGetSymbolAddress, with that device current) and
+ * caches it per device, so make one call per device before a capture starts.
+ *   events->n_events <= HEPF_SELECT_STATIC_MAX_EVENTS, otherwise HEPF_ERR_CAPACITY (hepf_last_error says so) and nothing
+ *   is launched.  Everything else — host/device placement, alignment, ownership, asynchrony on `stream` — as hepf_select.
+ * The array is shared by every call on that GPU and keeps the last call's contents.  Nothing in it has to start at zero
+ * (every word a call reads was written by the same call's select_eval_kernel), so it is not cleared; but two calls that
+ * OVERLAP on the GPU (different streams, or threads, without an ordering between them) race on it and give wrong
+ * survivor lists.  Calls on one stream, or ordered by events, are safe.
+ */
+#define HEPF_SELECT_STATIC_MAX_EVENTS 4194304 /* 2^22 events (BASELINE.json configs[1] has 4e6)                      */
+#define HEPF_SELECT_STATIC_BYTES 540928       /* = hepf_select_workspace_bytes(HEPF_SELECT_STATIC_MAX_EVENTS)         */
+int hepf_select_static(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
+                       int64_t* out_count, int64_t* out_cutflow, void* stream);
+
+/*
  * hepf_reconstruct_tth — for each listed event: for every smearing variation v < n_variations draw ten
  * standard normals from Philox4x32-10 keyed (seed; event_base+e, v, block) + Box-Muller, scale the two leptons
  * and the jets, propagate the change to the missing transverse momentum, and for every ordered pair of b-jet

@@ -70,6 +70,7 @@ def load():
         L.hepf_default_params.argtypes = [C.POINTER(Params)]
         L.hepf_select.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_void_p, C.c_size_t, C.c_void_p]
+        L.hepf_select_static.argtypes = [C.POINTER(_Events), C.POINTER(_Cut), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.hepf_reconstruct_tth.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_int64, C.c_int32, C.c_uint64,
                                            C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.hepf_reconstruct_tth_n.argtypes = [C.POINTER(_Events), C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_uint64,
@@ -198,6 +199,20 @@ def select(events: DeviceEvents, chain, *, with_cutflow: bool = True, out_idx=No
                        out_cutflow.data_ptr() if with_cutflow else None, ws.data_ptr(), ws.numel(), _stream_ptr(stream))
     _check(rc, "hepf_select")
     return out_idx, out_count, (out_cutflow[: len(chain)] if with_cutflow else None)
+
+
+SELECT_STATIC_MAX_EVENTS = 4194304   # HEPF_SELECT_STATIC_MAX_EVENTS (include/hepf.h)
+
+
+def select_static(events: DeviceEvents, chain, out_idx, out_count, out_cutflow=None, *, stream=None):
+    """hepf_select_static: hepf_select with its scratch in the library's static device array.  The entry point allocates
+    nothing, and neither does this wrapper: the caller passes every output (out_idx int32 [>= n_events], out_count int64 [1],
+    out_cutflow int64 [>= len(chain)] or None).  At most SELECT_STATIC_MAX_EVENTS events; calls that overlap on the GPU race."""
+    ev = events.view()
+    rc = load().hepf_select_static(C.byref(ev), make_cuts(chain), len(chain), out_idx.data_ptr(), out_count.data_ptr(),
+                                   out_cutflow.data_ptr() if out_cutflow is not None else None, _stream_ptr(stream))
+    _check(rc, "hepf_select_static")
+    return out_idx, out_count, (out_cutflow[: len(chain)] if out_cutflow is not None else None)
 
 
 def select_record(events: DeviceEvents, chain, derived_default: float = 0.0, *, with_cutflow: bool = True, ws=None, stream=None):

@@ -14,6 +14,8 @@
 //                      range from the 1-bit-per-event masks (1/1440 of K1's traffic) and writes the ascending
 //                      index list with popc-prefix offsets.  Deterministic, no atomics on the index cursor.
 // Each block owns a contiguous range of 512-event tiles; the grid is one wave of resident blocks (occupancy query: 2 per SM at 111 registers).
+#include <mutex>
+
 #include "hepf_common.cuh"
 
 namespace hepf {
@@ -449,6 +451,50 @@ extern "C" int hepf_select_record(const hepf_events_t* events, const hepf_cut_t*
                                   void* ws, size_t ws_bytes, void* stream_) {
   if (!out_derived) { set_error("hepf_select_record: out_derived is NULL"); return HEPF_ERR_ARG; }
   return select_impl(events, host_cuts, n_cuts, out_idx, out_count, out_cutflow, out_derived, derived_default, ws, ws_bytes,
+                     (cudaStream_t)stream_);
+}
+
+// ---- hepf_select_static: the same path with its scratch in a file-scope device array (include/hepf.h) ----------------------
+// In HOST code the name g_select_scratch is a host-side stand-in of the symbol, not a device address: what the kernels get is
+// the address cudaGetSymbolAddress returns, looked up once per device with that device current.
+constexpr size_t SELECT_STATIC_MASK_BYTES =
+    ((size_t)((HEPF_SELECT_STATIC_MAX_EVENTS + SEL_TILE - 1) / SEL_TILE + 1) * SEL_WARPS * sizeof(uint2) + 255) / 256 * 256;
+static_assert(SELECT_STATIC_MASK_BYTES + 4096 * sizeof(uint32_t) == HEPF_SELECT_STATIC_BYTES,
+              "HEPF_SELECT_STATIC_BYTES must equal hepf_select_workspace_bytes(HEPF_SELECT_STATIC_MAX_EVENTS)");
+static __device__ __align__(256) unsigned char g_select_scratch[HEPF_SELECT_STATIC_BYTES];
+
+constexpr int SELECT_STATIC_MAX_DEVICES = 64;
+static std::mutex g_select_scratch_lock;
+static void* g_select_scratch_addr[SELECT_STATIC_MAX_DEVICES] = {};
+
+static int select_static_scratch(void** addr) {
+  int dev = -1;
+  HEPF_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= SELECT_STATIC_MAX_DEVICES) { set_error("hepf_select_static: device ordinal %d not supported", dev); return HEPF_ERR_ARG; }
+  std::lock_guard<std::mutex> hold(g_select_scratch_lock);
+  if (!g_select_scratch_addr[dev]) {
+    void* p = nullptr;
+    HEPF_CUDA_TRY(cudaGetSymbolAddress(&p, g_select_scratch));
+    if (!p || !aligned(p, 256)) { set_error("hepf_select_static: bad address of the scratch array"); return HEPF_ERR_CUDA; }
+    g_select_scratch_addr[dev] = p;
+  }
+  *addr = g_select_scratch_addr[dev];
+  return HEPF_OK;
+}
+
+extern "C" int hepf_select_static(const hepf_events_t* events, const hepf_cut_t* host_cuts, int n_cuts, uint32_t* out_idx,
+                                  int64_t* out_count, int64_t* out_cutflow, void* stream_) {
+  int rc = check_events(events);
+  if (rc != HEPF_OK) return rc;
+  if (events->n_events > HEPF_SELECT_STATIC_MAX_EVENTS) {
+    set_error("hepf_select_static: %lld events exceed the static scratch (at most %d events; use hepf_select with a workspace)",
+              (long long)events->n_events, HEPF_SELECT_STATIC_MAX_EVENTS);
+    return HEPF_ERR_CAPACITY;
+  }
+  void* scratch = nullptr;
+  rc = select_static_scratch(&scratch);
+  if (rc != HEPF_OK) return rc;
+  return select_impl(events, host_cuts, n_cuts, out_idx, out_count, out_cutflow, nullptr, 0.0, scratch, HEPF_SELECT_STATIC_BYTES,
                      (cudaStream_t)stream_);
 }
 
