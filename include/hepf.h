@@ -238,7 +238,8 @@ size_t hepf_tth_host_arena_bytes(int64_t n_events, int32_t n_variations);
  * (b_lep, b_had, (q1, q2), solution), strict <.
  *   idx          device uint32[n_idx] events to reconstruct;  host_params NULL = (172.5, 80.4, 11.5, 7.5).
  *   out          device hepf_chi2_t[n_idx], 16-byte aligned.  status 1 = reconstructed, 2 = not applicable (n_lep != 1,
- *                fewer than 2 b-tagged or fewer than 2 untagged jets): NaN / -1 payload.
+ *                fewer than 2 b-tagged or fewer than 2 untagged jets): NaN / -1 payload.  A list entry idx[k] >= n_events
+ *                is not applicable with bit 8 set as well (status 10); nothing is read for it.
  */
 typedef struct { double m_top, m_w, sigma_top, sigma_w; } hepf_chi2_params_t;
 typedef struct {

@@ -19,7 +19,7 @@ constexpr int C2_THREADS = 128, C2_BLOCKS_PER_SM = 4;   // 40 KB of shared memor
 struct Chi2Cols {
   const double *lep_px, *lep_py, *lep_pz, *lep_e, *jet_px, *jet_py, *jet_pz, *jet_e, *met_x, *met_y;
   const uint32_t* flags;
-  int64_t stride;
+  int64_t n, stride;
 };
 struct P4 { double x, y, z, e; };
 __device__ __forceinline__ P4 add4(const P4& a, const P4& b) { return P4{a.x + b.x, a.y + b.y, a.z + b.z, a.e + b.e}; }
@@ -49,13 +49,20 @@ chi2_semilep_kernel(Chi2Cols ev, const uint32_t* __restrict__ idx, int64_t n_idx
   if (k >= n_idx) return;
   int64_t e = (int64_t)__ldg(idx + k);
   int64_t e1 = (k + step < n_idx) ? (int64_t)__ldg(idx + k + step) : 0;
-  uint32_t f = __ldg(ev.flags + e);
+  // a list entry beyond the store is "not applicable" (status 2 | 8) and nothing is read for it: its flags word is taken as 0
+  uint32_t f = ((uint64_t)e < (uint64_t)ev.n) ? __ldg(ev.flags + e) : 0u;
   for (;;) {
   const int64_t e2 = (k + 2 * step < n_idx) ? (int64_t)__ldg(idx + k + 2 * step) : 0;
-  const uint32_t f1 = (k + step < n_idx) ? __ldg(ev.flags + e1) : 0u;
+  const uint32_t f1 = (k + step < n_idx && (uint64_t)e1 < (uint64_t)ev.n) ? __ldg(ev.flags + e1) : 0u;
+  const bool in_range = (uint64_t)e < (uint64_t)ev.n;
+  const int64_t er = in_range ? e : 0;
   // lepton and MET go out together with the jets' copies below
-  const P4 lep{__ldg(ev.lep_px + e), __ldg(ev.lep_py + e), __ldg(ev.lep_pz + e), __ldg(ev.lep_e + e)};
-  const double nux = __ldg(ev.met_x + e), nuy = __ldg(ev.met_y + e);
+  P4 lep{0.0, 0.0, 0.0, 0.0};
+  double nux = 0.0, nuy = 0.0;
+  if (in_range) {
+    lep = P4{__ldg(ev.lep_px + er), __ldg(ev.lep_py + er), __ldg(ev.lep_pz + er), __ldg(ev.lep_e + er)};
+    nux = __ldg(ev.met_x + er); nuy = __ldg(ev.met_y + er);
+  }
   const int n_lep = f & 15u, n_jet = min(8u, (f >> 8) & 15u);
   // Candidate jets (the first <= 4 tagged and <= 4 untagged slots) are compacted into shared memory, one column of the block's
   // array per thread, by asynchronous 8-byte copies (cp.async: no register in between, so all <= 32 copies of an event are in
@@ -81,7 +88,7 @@ chi2_semilep_kernel(Chi2Cols ev, const uint32_t* __restrict__ idx, int64_t n_idx
   auto lj = [&](int i) { return P4{sj[0][i][0][tid], sj[0][i][1][tid], sj[0][i][2][tid], sj[0][i][3][tid]}; };
   hepf_chi2_t o;
   o.chi2 = o.nu_pz = o.m_top_lep = o.m_top_had = o.m_w_lep = o.m_w_had = CUDART_NAN;
-  o.jet_b_lep = o.jet_b_had = o.jet_q1 = o.jet_q2 = o.solution = -1; o.n_comb = 0; o.status = 2u; o.event = (uint32_t)e;
+  o.jet_b_lep = o.jet_b_had = o.jet_q1 = o.jet_q2 = o.solution = -1; o.n_comb = 0; o.status = in_range ? 2u : 10u; o.event = (uint32_t)e;
   if (n_lep == 1 && nbt >= (MODE == 0 ? 2 : 1) && (MODE == 1 || nlt >= 2)) {
     // ---- neutrino p_z from m(l nu) = m_W ---------------------------------------------------------------------------------
     const double ml2 = lep.e * lep.e - (lep.x * lep.x + lep.y * lep.y + lep.z * lep.z);
@@ -213,7 +220,7 @@ static int chi2_launch(const hepf_events_t* events, const uint32_t* idx, int64_t
   if (host_params) P = *host_params;
   if (!(P.sigma_top > 0.0) || !(P.sigma_w > 0.0)) { set_error("hepf_chi2: widths must be positive"); return HEPF_ERR_ARG; }
   const Chi2Cols cols{events->lep_px, events->lep_py, events->lep_pz, events->lep_e, events->jet_px, events->jet_py,
-                      events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags, events->stride};
+                      events->jet_pz, events->jet_e, events->met_x, events->met_y, events->flags, events->n_events, events->stride};
   int dev = 0, sms = 148;
   HEPF_CUDA_TRY(cudaGetDevice(&dev));
   HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));

@@ -709,6 +709,31 @@ def test_chi2_single_top_parity(hepf):
         hepf.chi2_single_top(dev, idx_t, 5, 0)
 
 
+def test_chi2_list_entries_beyond_the_store(hepf):
+    """idx[k] >= n_events: status 2 | 8, NaN / -1 payload, nothing read; every other record is unchanged (all three modes)."""
+    import torch
+    from paper_2211_14346_b200.binding import CHI2_DTYPE
+    st = hs.generate(5000, 61, semilep=True, with_truth=False)
+    dev = hepf.DeviceEvents.from_host(st)
+    idx = np.arange(st.n_events, dtype=np.uint32)
+    bad = idx.copy()
+    where = np.array([0, 31, 32, 1000, 4095, 4999])
+    bad[where] = [st.n_events, 2**32 - 1, st.n_events + 7, 2**31, st.stride, 2**32 - 2]
+    t = lambda a: torch.from_numpy(a.view(np.int32)).cuda()   # noqa: E731
+    for mode in (0, 1, 2):
+        run = (lambda i: hepf.chi2_semilep(dev, i, len(idx))) if mode == 0 else (lambda i: hepf.chi2_single_top(dev, i, len(idx), mode))
+        clean = run(t(idx)).cpu().numpy().reshape(-1).view(CHI2_DTYPE)
+        got = run(t(bad)).cpu().numpy().reshape(-1).view(CHI2_DTYPE)
+        keep = np.ones(len(idx), dtype=bool); keep[where] = False
+        assert got[keep].tobytes() == clean[keep].tobytes()
+        g = got[where]
+        assert (g["status"] == 10).all() and np.array_equal(g["event"], bad[where]) and (g["n_comb"] == 0).all()
+        assert np.isnan(g["chi2"]).all() and np.isnan(g["nu_pz"]).all() and (g["jet_b_lep"] == -1).all() and (g["solution"] == -1).all()
+    empty = hepf.DeviceEvents(torch.zeros((hs.NROW, 0), dtype=torch.float64, device="cuda"), torch.zeros(0, dtype=torch.int32, device="cuda"), 0, 0)
+    got = hepf.chi2_semilep(empty, t(idx[:40]), 40).cpu().numpy().reshape(-1).view(CHI2_DTYPE)     # an empty store: every entry is beyond it
+    assert (got["status"] == 10).all()
+
+
 def _chi2_dilep_compare(hepf, st, idx, par=None, split=None):
     import torch
     from paper_2211_14346_b200.binding import CHI2_DILEP_DTYPE
