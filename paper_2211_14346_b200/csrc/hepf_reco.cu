@@ -493,27 +493,37 @@ __device__ __noinline__ bool polish_raw(const V4 lp, const V4 bi, const V4 lm, c
     A[1][0] = 2.0 * (s2 * ux - (lp.x + bi.x)); A[1][1] = 2.0 * (s2 * uy - (lp.y + bi.y)); A[1][2] = 2.0 * (s2 * uz - (lp.z + bi.z)); A[1][3] = 0.0;
     A[2][0] = -2.0 * (t1 * vx - lm.x); A[2][1] = -2.0 * (t1 * vy - lm.y); A[2][2] = 0.0; A[2][3] = 2.0 * (t1 * vz - lm.z);
     A[3][0] = -2.0 * (t2 * vx - (lm.x + bj.x)); A[3][1] = -2.0 * (t2 * vy - (lm.y + bj.y)); A[3][2] = 0.0; A[3][3] = 2.0 * (t2 * vz - (lm.z + bj.z));
-    // Gaussian elimination with partial pivoting (rows swapped in place); the step only has to be good to a few digits
+    // Gaussian elimination with partial pivoting; the step only has to be good to a few digits.  Every index is a compile-time
+    // constant (the pivot row is brought up by conditional swaps of whole rows), so the matrix stays in registers.
     double ipv[4];
+#pragma unroll
     for (int c = 0; c < 4; c++) {
-      int pr = c;
-      for (int r = c + 1; r < 4; r++) if (fabs(A[r][c]) > fabs(A[pr][c])) pr = r;
-      for (int k = 0; k < 5; k++) { const double t = A[c][k]; A[c][k] = A[pr][k]; A[pr][k] = t; }
+#pragma unroll
+      for (int r = c + 1; r < 4; r++) {
+        const bool sw = fabs(A[r][c]) > fabs(A[c][c]);
+#pragma unroll
+        for (int k = c; k < 5; k++) { const double t = A[c][k]; A[c][k] = sw ? A[r][k] : t; A[r][k] = sw ? t : A[r][k]; }
+      }
       ipv[c] = rcp_fast(A[c][c]);
+#pragma unroll
       for (int r = c + 1; r < 4; r++) {
         const double m = A[r][c] * ipv[c];
-        for (int k = c; k < 5; k++) A[r][k] -= m * A[c][k];
+#pragma unroll
+        for (int k = c + 1; k < 5; k++) A[r][k] -= m * A[c][k];
       }
     }
     double d[4];
+#pragma unroll
     for (int c = 3; c >= 0; c--) {
       double sacc = A[c][4];
+#pragma unroll
       for (int k = c + 1; k < 4; k++) sacc -= A[c][k] * d[k];
       d[c] = sacc * ipv[c];
     }
     mv = fabs(d[0]) + fabs(d[1]) + fabs(d[2]) + fabs(d[3]);
     total += mv;
     if (!(total <= 1e-3 * scale)) return false;     // NaN, or wandering off to another intersection
+#pragma unroll
     for (int c = 0; c < 4; c++) u[c] = dd_sub(u[c], DD{d[c], 0.0});
   }
   if (!(mv <= 1e-10 * scale)) return false;
@@ -1030,13 +1040,21 @@ reco_search_kernel(RecoCols ev, const uint32_t* __restrict__ idx, const int64_t*
   }
 }
 
+constexpr int FIN_THREADS = 128;
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gmem_src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 // One selected event: re-derive the winner in full, polish it and write the record.
 __device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_t* __restrict__ idx, int64_t k, int64_t n_cap, uint32_t k0,
                                                uint32_t k1, const hepf_tth_params_t& P, const uint2* __restrict__ winners,
-                                               const double* __restrict__ nominal, hepf_best_t* __restrict__ out) {
+                                               const double* __restrict__ nominal, hepf_best_t* __restrict__ out,
+                                               double (*__restrict__ s_obj)[FIN_THREADS]) {
   const EventHead h = load_head(ev, (int64_t)__ldg(idx + k));
   const uint2 w = winners[k];
   hepf_best_t* o = out + k;
+  const int tid = threadIdx.x;
   if (!h.applicable || !w.y) {
     const double n = CUDART_NAN;
     o->nu[0] = o->nu[1] = o->nu[2] = o->nubar[0] = o->nubar[1] = o->nubar[2] = n;
@@ -1050,57 +1068,14 @@ __device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_
   const double mt2 = P.m_top * P.m_top, mw2 = P.m_w * P.m_w, inv_lambda = rcp_fast(P.lambda_nu), inv_sh = rcp_fast(P.sigma_higgs);
   // Nominal objects and MET from the workspace copy the search kernel left (42 columns of n_cap doubles: consecutive
   // threads read consecutive addresses), not from the store, where every value of a selected event is its own DRAM atom.
-  double obj[10][4], sc[10], ksv[10];
+  // The 40 object components go straight into this thread's column of the block's shared array (cp.async: all in flight
+  // together, no register in between): they are indexed by jet slot further down, and as a thread-local array they were
+  // 0.9 KB of local memory per thread that left L2 (0.57 GB of DRAM writes per launch on cfg4).
 #pragma unroll
-  for (int t = 0; t < 10; t++)
-#pragma unroll
-    for (int c = 0; c < 4; c++) obj[t][c] = __ldcs(nominal + (int64_t)(4 * t + c) * n_cap + k);
+  for (int it = 0; it < 40; it++) cp_async8(&s_obj[it][tid], nominal + (int64_t)it * n_cap + k);
   const double met_x = __ldcs(nominal + 40 * n_cap + k), met_y = __ldcs(nominal + 41 * n_cap + k);
-#pragma unroll
-  for (int t = 0; t < 10; t++) {       // kappa * sigma as load_object computes it (step 2)
-    const double sigma = t < 2 ? P.lep_sigma : __dadd_rn(__ddiv_rn(P.jet_stoch, __dsqrt_rn(obj[t][3])), P.jet_const);
-    ksv[t] = t < 2 + h.n_jet ? __dmul_rn(P.sigma_scale, sigma) : 0.0;
-  }
-  // smear this variation
-  double ax = 0.0, ay = 0.0;
-  for (int blk = 0; blk < h.nblk; blk++) {
-    uint32_t x[4];
-    philox4x32_10((uint32_t)h.gidx, (uint32_t)(h.gidx >> 32), (uint32_t)v, 0x54544800u + blk, k0, k1, x);
-    double z[2]; block_normals(x, z[0], z[1]);
-    for (int u = 0; u < 2; u++) {
-      const int t = 2 * blk + u;
-      sc[t] = scale_of(ksv[t], z[u], P.s_min);
-      if (t < 2 + h.n_jet) {
-        const double d = __dadd_rn(sc[t], -1.0);
-        ax = __dadd_rn(ax, __dmul_rn(d, obj[t][0])); ay = __dadd_rn(ay, __dmul_rn(d, obj[t][1]));
-      }
-    }
-  }
-  const double Mx = __dadd_rn(met_x, -ax), My = __dadd_rn(met_y, -ay);
   const int lps = h.lp_slot, lms = 1 - h.lp_slot;
   const int si = (h.cand >> (4 * i)) & 15, sj = (h.cand >> (4 * j)) & 15;
-  const V4 lp = scale_v4(obj[lps], sc[lps]), lm = scale_v4(obj[lms], sc[lms]);
-  const V4 bi = scale_v4(obj[2 + si], sc[2 + si]), bj = scale_v4(obj[2 + sj], sc[2 + sj]);
-  // same frame-based construction as the search kernel (identical bits)
-  const double hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2);
-  const Frame F1 = make_frame(obj[lps], obj[2 + si]), F2 = make_frame(obj[lms], obj[2 + sj]);
-  Conic A, q2; double c0, e0;
-  A.a = F1.a; A.b = F1.b; A.c = F1.c; q2.a = F2.a; q2.b = F2.b; q2.c = F2.c;
-  conic_def(F1, sc[lps], sc[2 + si], rcp_fast(sc[lps]), rcp_fast(sc[2 + si]), hmw2, hcm, c0, A.d, A.e, A.f);
-  conic_def(F2, sc[lms], sc[2 + sj], rcp_fast(sc[lms]), rcp_fast(sc[2 + sj]), hmw2, hcm, e0, q2.d, q2.e, q2.f);
-  const double c1 = F1.c1, c2 = F1.c2, e1 = F2.c1, e2 = F2.c2;
-  const Conic B = shift_conic(q2, Mx, My);
-  double g3, g2, g1, g0, xa[2] = {0, 0}, xb[2] = {0, 0};
-  resultant(A, B, pair_consts(A.a, A.b, A.c, B.a, B.b, B.c), g3, g2, g1, g0);
-  const int mask = solve_quartic(g3, g2, g1, g0, seed_scale(P), xa, xb);
-  double xs[4], ys[4]; int nr = 0;
-  if (mask & 1) { xs[0] = xa[0]; xs[1] = xa[1]; nr = 2; }
-  if (mask & 2) { xs[nr] = xb[0]; xs[nr + 1] = xb[1]; nr += 2; }
-  for (int r = 0; r < nr; r++) refine_xy<false>(A, B, xs[r], ys[r]);
-  const int rs = ksel < nr ? ksel : 0;
-  const double xx = nr ? xs[rs] : CUDART_NAN, yy = nr ? ys[rs] : CUDART_NAN;
-  int rank = 0;
-  for (int r = 0; r < nr; r++) rank += (xs[r] < xx) || (xs[r] == xx && r < rs);
   // Higgs pair hsel among the candidates not used by (i, j)
   int hk = 0, hl = 1, hc = 0;
   for (int kk = 0; kk < nb; kk++) for (int l = kk + 1; l < nb; l++) {
@@ -1109,7 +1084,71 @@ __device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_
     hc++;
   }
   const int sh1 = (h.cand >> (4 * hk)) & 15, sh2 = (h.cand >> (4 * hl)) & 15;
-  const V4 h1 = scale_v4(obj[2 + sh1], sc[2 + sh1]), h2 = scale_v4(obj[2 + sh2], sc[2 + sh2]);
+  cp_async_wait_all();
+  auto obj4 = [&](int t, double (&p)[4]) {
+#pragma unroll
+    for (int c = 0; c < 4; c++) p[c] = s_obj[4 * t + c][tid];
+  };
+  // smear this variation: every scale enters the MET, six of them (the two leptons, b, bbar and the Higgs pair) are kept
+  double ax = 0.0, ay = 0.0;
+  double sc_lp = 1.0, sc_lm = 1.0, sc_bi = 1.0, sc_bj = 1.0, sc_h1 = 1.0, sc_h2 = 1.0;
+  for (int blk = 0; blk < h.nblk; blk++) {
+    uint32_t x[4];
+    philox4x32_10((uint32_t)h.gidx, (uint32_t)(h.gidx >> 32), (uint32_t)v, 0x54544800u + blk, k0, k1, x);
+    double z[2]; block_normals(x, z[0], z[1]);
+#pragma unroll
+    for (int u = 0; u < 2; u++) {
+      const int t = 2 * blk + u;
+      // kappa * sigma as load_object computes it (step 2)
+      const double sigma = t < 2 ? P.lep_sigma : __dadd_rn(__ddiv_rn(P.jet_stoch, __dsqrt_rn(s_obj[4 * t + 3][tid])), P.jet_const);
+      const double ks = t < 2 + h.n_jet ? __dmul_rn(P.sigma_scale, sigma) : 0.0;
+      const double sct = scale_of(ks, z[u], P.s_min);
+      if (t < 2 + h.n_jet) {
+        const double d = __dadd_rn(sct, -1.0);
+        ax = __dadd_rn(ax, __dmul_rn(d, s_obj[4 * t][tid])); ay = __dadd_rn(ay, __dmul_rn(d, s_obj[4 * t + 1][tid]));
+      }
+      sc_lp = t == lps ? sct : sc_lp; sc_lm = t == lms ? sct : sc_lm;
+      sc_bi = t == 2 + si ? sct : sc_bi; sc_bj = t == 2 + sj ? sct : sc_bj;
+      sc_h1 = t == 2 + sh1 ? sct : sc_h1; sc_h2 = t == 2 + sh2 ? sct : sc_h2;
+    }
+  }
+  const double Mx = __dadd_rn(met_x, -ax), My = __dadd_rn(met_y, -ay);
+  double o_lp[4], o_lm[4], o_bi[4], o_bj[4];
+  obj4(lps, o_lp); obj4(lms, o_lm); obj4(2 + si, o_bi); obj4(2 + sj, o_bj);
+  const V4 lp = scale_v4(o_lp, sc_lp), lm = scale_v4(o_lm, sc_lm);
+  const V4 bi = scale_v4(o_bi, sc_bi), bj = scale_v4(o_bj, sc_bj);
+  // same frame-based construction as the search kernel (identical bits)
+  const double hmw2 = 0.5 * mw2, hcm = 0.5 * (mt2 - mw2);
+  const Frame F1 = make_frame(o_lp, o_bi), F2 = make_frame(o_lm, o_bj);
+  Conic A, q2; double c0, e0;
+  A.a = F1.a; A.b = F1.b; A.c = F1.c; q2.a = F2.a; q2.b = F2.b; q2.c = F2.c;
+  conic_def(F1, sc_lp, sc_bi, rcp_fast(sc_lp), rcp_fast(sc_bi), hmw2, hcm, c0, A.d, A.e, A.f);
+  conic_def(F2, sc_lm, sc_bj, rcp_fast(sc_lm), rcp_fast(sc_bj), hmw2, hcm, e0, q2.d, q2.e, q2.f);
+  const double c1 = F1.c1, c2 = F1.c2, e1 = F2.c1, e2 = F2.c2;
+  const Conic B = shift_conic(q2, Mx, My);
+  double g3, g2, g1, g0, xa[2] = {0, 0}, xb[2] = {0, 0};
+  resultant(A, B, pair_consts(A.a, A.b, A.c, B.a, B.b, B.c), g3, g2, g1, g0);
+  const int mask = solve_quartic(g3, g2, g1, g0, seed_scale(P), xa, xb);
+  // the <= 4 roots: x in registers (static indices), refined one by one; the selected one is kept on the way
+  const bool ma = mask & 1, mb = mask & 2;
+  const int nr = (ma ? 2 : 0) + (mb ? 2 : 0);
+  const double xs[4] = {ma ? xa[0] : xb[0], ma ? xa[1] : xb[1], xb[0], xb[1]};
+  const int rs = ksel < nr ? ksel : 0;
+  double xx = CUDART_NAN, yy = CUDART_NAN;
+  double xr[4];
+#pragma unroll 1
+  for (int r = 0; r < nr; r++) {
+    double x = r == 0 ? xs[0] : r == 1 ? xs[1] : r == 2 ? xs[2] : xs[3], y;
+    refine_xy<false>(A, B, x, y);
+    if (r == rs) { xx = x; yy = y; }
+    if (r == 0) xr[0] = x; else if (r == 1) xr[1] = x; else if (r == 2) xr[2] = x; else xr[3] = x;
+  }
+  int rank = 0;
+#pragma unroll
+  for (int r = 0; r < 4; r++) if (r < nr) rank += (xr[r] < xx) || (xr[r] == xx && r < rs);
+  double o_h1[4], o_h2[4];
+  obj4(2 + sh1, o_h1); obj4(2 + sh2, o_h2);
+  const V4 h1 = scale_v4(o_h1, sc_h1), h2 = scale_v4(o_h2, sc_h2);
   const double mbb = mass_of(h1.e + h2.e, h1.x + h2.x, h1.y + h2.y, h1.z + h2.z);
   const double t = (mbb - P.m_higgs) * inv_sh, ht = -0.5 * (t * t);
   double pz = fma(c2, yy, fma(c1, xx, c0));
@@ -1132,13 +1171,14 @@ __device__ __forceinline__ void finalize_event(const RecoCols& ev, const uint32_
 }
 
 // One thread per listed event (grid-stride: the grid is sized from the capacity, the length may live on the device).
-__global__ void __launch_bounds__(128, 4)   // 128 registers: the kernel is a chain of dependent FP64 operations, more resident warps hide it
+__global__ void __launch_bounds__(FIN_THREADS, 4)   // 128 registers: the kernel is a chain of dependent FP64 operations, more resident warps hide it
 reco_finalize_kernel(RecoCols ev, const uint32_t* __restrict__ idx, const int64_t* __restrict__ n_dev, int64_t n_cap, uint32_t k0,
                      uint32_t k1, hepf_tth_params_t P, const uint2* __restrict__ winners, const double* __restrict__ nominal,
                      hepf_best_t* __restrict__ out) {
+  __shared__ double s_obj[40][FIN_THREADS];   // a column per thread: the nominal objects of its event (40 KB per block)
   const int64_t n_idx = list_length(n_dev, n_cap);
-  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_idx; k += (int64_t)gridDim.x * blockDim.x)
-    finalize_event(ev, idx, k, n_cap, k0, k1, P, winners, nominal, out);
+  for (int64_t k = (int64_t)blockIdx.x * FIN_THREADS + threadIdx.x; k < n_idx; k += (int64_t)gridDim.x * FIN_THREADS)
+    finalize_event(ev, idx, k, n_cap, k0, k1, P, winners, nominal, out, s_obj);
 }
 
 // hepf_tth_system: invariant mass and transverse momentum of the reconstructed ttH system of each record (PAPER.md:410-442,
@@ -1289,7 +1329,7 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, con
   // chunk of variations per pass of the pipeline: 32 when that wastes at most an eighth of the lanes of the last chunk,
   // else 16 or 8.  32 (16 for n_b = 6) needs so much shared memory per warp that one block of 18 (19) warps fills an SM.
   const int waste32 = ((n_variations + 31) & ~31) - n_variations;
-  if (n_variations <= 2) rc = launch_search_both<1, 1, 2, 2, 10, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);   // lanes = pairings
+  if (n_variations <= 2) rc = launch_search_both<1, 1, 2, 2, 16, 16>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);   // lanes = pairings
   else if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 2, 12, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
   else if (8 * waste32 > n_variations) rc = launch_search_both<16, 8, 2, 2, 10, 9>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
   else rc = launch_search_both<32, 16, 18, 19, 1, 1>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
@@ -1298,7 +1338,7 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, con
   HEPF_CUDA_TRY(cudaGetDevice(&dev));
   HEPF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   const int64_t want = (n_idx + 127) / 128, cap = (int64_t)sms * 32;
-  reco_finalize_kernel<<<(unsigned)(want < cap ? want : cap), 128, 0, stream>>>(cols, idx, n_dev, n_idx, (uint32_t)seed,
+  reco_finalize_kernel<<<(unsigned)(want < cap ? want : cap), FIN_THREADS, 0, stream>>>(cols, idx, n_dev, n_idx, (uint32_t)seed,
                                                                              (uint32_t)(seed >> 32), P, winners, nominal, out_best);
   count_launch();
   timing_mark(T_RECO3, stream);
