@@ -1331,7 +1331,7 @@ int hepf::reconstruct_impl(const hepf_events_t* events, const uint32_t* idx, con
   const int waste32 = ((n_variations + 31) & ~31) - n_variations;
   if (n_variations <= 2) rc = launch_search_both<1, 1, 2, 2, 16, 16>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);   // lanes = pairings
   else if (n_variations <= 8) rc = launch_search_both<8, 8, 2, 2, 12, 10>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
-  else if (8 * waste32 > n_variations) rc = launch_search_both<16, 8, 2, 2, 10, 9>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
+  else if (8 * waste32 > n_variations) rc = launch_search_both<16, 8, 3, 2, 7, 9>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
   else rc = launch_search_both<32, 16, 18, 19, 1, 1>(cols, idx, n_dev, n_idx, n_variations, seed, P, winners, nominal, stream);
   if (rc != HEPF_OK) return rc;
   int dev = 0, sms = 148;
