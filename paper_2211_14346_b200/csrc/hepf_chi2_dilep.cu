@@ -51,7 +51,7 @@ __device__ __forceinline__ int nu_pz(const Q4& l, double hmw2ml, double a, doubl
 
 // One leg at one grid point: for every candidate b the smaller of the (up to two) terms and which solution gave it.
 struct LegMin { double v[4]; int s[4]; };
-__device__ __forceinline__ LegMin leg_min(const Q4& l, const Q4 (&b)[4], int nbt, int nsol, const double (&pz)[2], double nux, double nuy,
+__device__ __forceinline__ LegMin leg_min(const Q4& l, const Q4* __restrict__ b, int nbt, int nsol, const double (&pz)[2], double nux, double nuy,
                                           double m_top, double m_w, double ist, double isw) {
   LegMin L;
 #pragma unroll
@@ -78,7 +78,7 @@ __device__ __forceinline__ LegMin leg_min(const Q4& l, const Q4 (&b)[4], int nbt
 
 __device__ __forceinline__ double grid_u(int g, double gn) { return (double)(2 * g + 1) / gn - 1.0; }
 
-__global__ void __launch_bounds__(32 * CD_WARPS, 5)   // 96 registers, 20 warps per SM: the dependent FP64 chains want the occupancy (164 registers unbounded: 11.3 vs 9.5 ms)
+__global__ void __launch_bounds__(32 * CD_WARPS, 6)   // 80 registers, 24 warps per SM: the dependent FP64 chains want the occupancy (164 registers unbounded: 11.3 ms; 96 registers / 20 warps: 9.5 ms; this: 9.2 ms)
 chi2_dilep_kernel(DilepCols ev, const uint32_t* __restrict__ idx, int64_t n_idx, hepf_chi2_params_t P, double split_range,
                   int G, hepf_chi2_dilep_t* __restrict__ out) {
   const int lane = threadIdx.x & 31;
@@ -105,12 +105,16 @@ chi2_dilep_kernel(DilepCols ev, const uint32_t* __restrict__ idx, int64_t n_idx,
   const int lp = q0 ? 0 : 1, lm = 1 - lp;
   const Q4 lplus{__ldg(ev.lep_px + lp * ev.stride + e), __ldg(ev.lep_py + lp * ev.stride + e), __ldg(ev.lep_pz + lp * ev.stride + e), __ldg(ev.lep_e + lp * ev.stride + e)};
   const Q4 lminus{__ldg(ev.lep_px + lm * ev.stride + e), __ldg(ev.lep_py + lm * ev.stride + e), __ldg(ev.lep_pz + lm * ev.stride + e), __ldg(ev.lep_e + lm * ev.stride + e)};
-  Q4 b[4];
-#pragma unroll
-  for (int c = 0; c < 4; c++) {
-    const int64_t at = (int64_t)bt[c] * ev.stride + e;
-    b[c] = c < nbt ? Q4{__ldg(ev.jet_px + at), __ldg(ev.jet_py + at), __ldg(ev.jet_pz + at), __ldg(ev.jet_e + at)} : Q4{0.0, 0.0, 0.0, 0.0};
+  // The candidate b jets are the same for every lane of the warp: they sit in shared memory (broadcast reads in the scan),
+  // not in 32 registers of every thread.
+  __shared__ Q4 s_b[CD_WARPS][4];
+  Q4* b = s_b[threadIdx.x >> 5];
+  if (lane < 4) {
+    const int slot = lane == 0 ? bt[0] : lane == 1 ? bt[1] : lane == 2 ? bt[2] : bt[3];
+    const int64_t at = (int64_t)slot * ev.stride + e;
+    b[lane] = lane < nbt ? Q4{__ldg(ev.jet_px + at), __ldg(ev.jet_py + at), __ldg(ev.jet_pz + at), __ldg(ev.jet_e + at)} : Q4{0.0, 0.0, 0.0, 0.0};
   }
+  __syncwarp();
   const double Mx = __ldg(ev.met_x + e), My = __ldg(ev.met_y + e);
   const double ist = rcp_fast(P.sigma_top), isw = rcp_fast(P.sigma_w), gn = (double)G;
   const double ml2p = lplus.e * lplus.e - (lplus.x * lplus.x + lplus.y * lplus.y + lplus.z * lplus.z);
